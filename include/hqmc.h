@@ -1,0 +1,142 @@
+/*
+ * hqmc.h -- C ABI of libhqmc.so: the pseudofermion hot path of the hybrid quantum Monte Carlo
+ * method of arxiv/paper_2508_16298 ("Scalable hybrid quantum Monte Carlo simulation of U(1) gauge
+ * field coupled to fermions on GPU"), hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations are to /root/reference/PAPER.md (line numbers) and to the readings C1-C22 listed in
+ * DESIGN.md (taken from SURVEY.md section 8c).
+ *
+ * Conventions (all entry points)
+ *  - Lattice: L x L sites per time slice (L even, >= 4), Ntau >= 2 slices, N = Ntau*L*L sites.
+ *    Site s = x + L*y.  Vector element (tau, s) lives at index tau*L*L + s, interleaved (re, im):
+ *    complex128 for HQMC_C128, complex64 for HQMC_C64.
+ *  - Gauge field theta (and momentum p, and dS/dtheta): always fp64, layout [Ntau][2][L][L]:
+ *    bond (tau, mu, s) at (tau*2 + mu)*L*L + s; mu = 0: s -> s + x, mu = 1: s -> s + y, periodic in
+ *    space (Eq.1, 46 Fig.1; reading C3: matrix element (i, j) of a bond i -> j is
+ *    e^{+i theta}).  Temporal links are fixed to 0.
+ *  - Pointers named d_* are DEVICE pointers, 16-byte aligned, owned by the caller; pointers named
+ *    h_* / *_out are HOST pointers.  The library never frees or keeps caller memory beyond the call
+ *    (hqmc_set_theta copies theta into the context).  `in` and `out` must not alias unless marked
+ *    in/out.
+ *  - All work is enqueued on the CUDA stream given to hqmc_create.  Calls with host out-parameters
+ *    (hqmc_cg_solve, hqmc_leapfrog_trajectory, hqmc_energies, *_host) synchronise that stream
+ *    before returning; the others return as soon as the work is enqueued.
+ *  - Return value: 0 on success, negative hqmc_status otherwise.  No exceptions, no exit(), no CPU
+ *    fallback: without a CUDA device every compute call returns HQMC_ECUDA.
+ */
+#ifndef HQMC_H
+#define HQMC_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hqmc_ctx hqmc_ctx; /* opaque: phase table, theta copy, CG workspace, reduction scratch, graphs */
+
+typedef enum { HQMC_C128 = 0, HQMC_C64 = 1 } hqmc_prec;
+
+typedef enum {
+    HQMC_OK = 0,
+    HQMC_EINVAL = -1,  /* bad argument: odd L, L < 4, Ntau < 2, null or misaligned pointer, bad W   */
+    HQMC_ECUDA = -2,   /* CUDA error (text via hqmc_last_error)                                    */
+    HQMC_ENOCONV = -3, /* CG hit max_iter above tol; x, iters_out, relres_out are still valid      */
+    HQMC_ENOMEM = -4   /* device allocation failed                                                 */
+} hqmc_status;
+
+typedef struct {
+    int L, Ntau;       /* L even >= 4; Ntau >= 2.  Paper: Ntau = 10 L                 */
+    double dtau, t;    /* Trotter step 0.1 and hopping 1                         */
+    double c_tau, K;   /* S_B couplings: c_tau = 1/(J dtau^2), K (reading C12)     */
+    int compact;       /* 1: compact L_B^c; 0: non-compact L_B^nc (Eq.2) */
+    int precond_W;     /* preconditioner half bandwidth in tau, 0..32; 0 = identity (reading C10)  */
+    hqmc_prec prec;    /* arithmetic of the fermion vectors                                        */
+} hqmc_params;
+
+/* Create a context for one lattice.  cuda_stream is a cudaStream_t (NULL = legacy default stream).
+ * Allocates the workspace (phase table, theta copy, 5 CG vectors, scratch) and, if precond_W > 0,
+ * builds the default preconditioner taps on the device from the library's own B at pi-flux
+ * (reading C10: c_k = [B_pi^k]_00, p_m = sum_k c_k c_{k+m}). */
+int hqmc_create(const hqmc_params *params, void *cuda_stream, hqmc_ctx **out);
+int hqmc_destroy(hqmc_ctx *ctx);
+
+/* Override the preconditioner: z_{tau,i} = sum_{m=-W..W} taps[|m|] s(tau,m) r_{tau+m,i}, s = -1 when
+ * tau+m wraps (antiperiodic fermions).  taps_host has W+1 entries (host memory). */
+int hqmc_set_precond(hqmc_ctx *ctx, int W, const double *taps_host);
+/* Read back the taps in use (host array of at least 33 doubles); *W_out receives W. */
+int hqmc_get_precond(hqmc_ctx *ctx, int *W_out, double *taps_host);
+
+/* Copy theta [Ntau][2][L][L] (device, fp64) into the context and rebuild the link-phase table
+ * e^{i theta} (scaled per bond family, Eq.22-26).  Must precede apply/solve/force. */
+int hqmc_set_theta(hqmc_ctx *ctx, const double *d_theta);
+
+/* Matrix-free fermion matrix (Eq.8; reading C1; 0-based slices), with
+ * B_tau = e^{V4/2} e^{V3/2} e^{V2/2} e^{V1} e^{V2/2} e^{V3/2} e^{V4/2} (Eq.22, reading C5):
+ *   (M v)_t    = v_t - B_{t-1} v_{t-1} (t >= 1),   (M v)_0       = v_0 + B_{Nt-1} v_{Nt-1}
+ *   (M^+ w)_t  = w_t - B_t w_{t+1}   (t < Nt-1),  (M^+ w)_{Nt-1} = w_{Nt-1} + B_{Nt-1} w_0
+ * hqmc_apply_MdagM is the fused O = M^+ M of PAPER.md:248, 284-314. */
+int hqmc_apply_M(hqmc_ctx *ctx, const void *d_in, void *d_out);
+int hqmc_apply_Mdag(hqmc_ctx *ctx, const void *d_in, void *d_out);
+int hqmc_apply_MdagM(hqmc_ctx *ctx, const void *d_in, void *d_out);
+
+/* Banded preconditioner O~^{-1} r (reading C10). */
+int hqmc_precond(hqmc_ctx *ctx, const void *d_in, void *d_out);
+
+/* Preconditioned CG on M^+M x = rhs (Eq.20; readings C8, C9): x_0 = 0, d_0 = P r_0,
+ * stop when ||r_n|| / ||rhs|| <= tol (recurrence residual, tested after the r update).
+ * tol <= 0: run exactly max_iter iterations (the paper's fixed-count CUDA-graph mode).
+ * iters_out / relres_out (host, may be NULL): iterations done and ||r|| / ||rhs|| at exit. */
+int hqmc_cg_solve(hqmc_ctx *ctx, const void *d_rhs, void *d_x, double tol, long long max_iter,
+                  long long *iters_out, double *relres_out);
+
+/* Fermionic force dS_F/dtheta for S_F = phi^+ (M^+M)^{-1} phi, given x = (M^+M)^{-1} phi
+ * (PAPER.md:455-477 SI; reading C11): dS_F/dtheta_{b,t} = 2 sigma_t Re[ Y_{t+1}^+ (dB_t/dtheta_b) x_t ],
+ * Y = M x.  Output fp64 [Ntau][2][L][L]. */
+int hqmc_force(hqmc_ctx *ctx, const void *d_x, double *d_dSF_dtheta);
+
+/* Bosonic force dS_B/dtheta at the context's theta.  Output as above. */
+int hqmc_force_boson(hqmc_ctx *ctx, double *d_dSB_dtheta);
+
+/* Energies at the context's theta: S_B(theta); sum p^2 (if d_p != NULL); S_F = Re <phi, x>
+ * (if d_phi and d_x != NULL) (Eq.12).  Host outputs, any may be NULL. */
+int hqmc_energies(hqmc_ctx *ctx, const double *d_p, const void *d_phi, const void *d_x, double *SB_out,
+                  double *p2_out, double *SF_out);
+
+/* One molecular-dynamics trajectory of nsteps leapfrog steps (Eq.16; reading C7):
+ *   p += F eps/2;  theta += 2 p eps;  p += F eps/2,   F = -dS_B/dtheta - dS_F/dtheta,
+ * with H = S_B + sum p^2 + phi^+ (M^+M)^{-1} phi (Eq.12): nsteps + 1 CG solves.
+ * d_theta, d_p: in/out (fp64 [Ntau][2][L][L]); d_pf: the pseudofermion phi.  H0_out / H1_out: H at
+ * the start / end; cg_iters_out: total CG iterations (host, may be NULL).
+ * Returns HQMC_ENOCONV if any solve hit cg_max_iter with cg_tol > 0 (results still written). */
+int hqmc_leapfrog_trajectory(hqmc_ctx *ctx, double *d_theta, double *d_p, const void *d_pf, int nsteps,
+                             double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
+                             long long *cg_iters_out);
+
+/* HOST-buffer variants (pageable or pinned host memory; the copies run inside the call on the
+ * context's stream and the call returns after the result has landed in h_out / h_x). */
+int hqmc_apply_MdagM_host(hqmc_ctx *ctx, const void *h_in, void *h_out);
+int hqmc_cg_solve_host(hqmc_ctx *ctx, const double *h_theta, const void *h_rhs, void *h_x, double tol,
+                       long long max_iter, long long *iters_out, double *relres_out);
+int hqmc_leapfrog_trajectory_host(hqmc_ctx *ctx, double *h_theta, double *h_p, const void *h_pf, int nsteps,
+                                  double eps, double cg_tol, long long cg_max_iter, double *H0_out,
+                                  double *H1_out, long long *cg_iters_out);
+
+/* Instrumentation.  hqmc_set_profiling(ctx, 1) makes the library bracket each launch of its kernels
+ * with CUDA events on the context's stream (CG then runs without graph replay); hqmc_get_kernel_stats
+ * returns, for kernel class `which` (HQMC_K_*), the number of launches and the summed device time in
+ * ms since the last hqmc_reset_stats.  Launch counts are kept even when profiling is off. */
+enum { HQMC_K_MDAGM = 0, HQMC_K_AXPY = 1, HQMC_K_PRECOND = 2, HQMC_K_DUPDATE = 3, HQMC_K_M = 4,
+       HQMC_K_FORCE = 5, HQMC_K_PHASE = 6, HQMC_K_MISC = 7, HQMC_K_COUNT = 8 };
+int hqmc_set_profiling(hqmc_ctx *ctx, int on);
+int hqmc_reset_stats(hqmc_ctx *ctx);
+int hqmc_get_kernel_stats(hqmc_ctx *ctx, int which, long long *launches_out, double *ms_out);
+/* Tuning knob: slices per CTA of the fused M^+M kernel (0 = library default). */
+int hqmc_set_time_tile(hqmc_ctx *ctx, int slices_per_cta);
+
+const char *hqmc_strerror(int status);
+const char *hqmc_last_error(void); /* text of the last CUDA error seen by this thread, or "" */
+int hqmc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HQMC_H */

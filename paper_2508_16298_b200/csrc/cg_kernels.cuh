@@ -1,0 +1,152 @@
+// cg_kernels.cuh -- preconditioned CG pieces (Eq.20; readings C8, C9) and the
+// tau-banded preconditioner (reading C10).
+//
+// Reductions are single pass: every producer CTA writes ONE partial; every consumer CTA re-sums the
+// partials in a fixed order (warp 0: lane-strided adds + shuffle tree), so alpha/beta are bitwise equal
+// in all CTAs, run-to-run deterministic, with no atomics, no extra kernel and no host round trip.
+#pragma once
+#include "kernels.cuh"
+
+namespace hqmc {
+
+// x = 0, r = rhs, part_rr[b] = partial ||rhs||^2
+template <typename T>
+__global__ void k_cg_init(size_t N, const typename Cx<T>::type *__restrict__ rhs, typename Cx<T>::type *__restrict__ x,
+                          typename Cx<T>::type *__restrict__ r, double *__restrict__ part_rr) {
+    typedef typename Cx<T>::type T2;
+    __shared__ double red[32];
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        T2 b = rhs[i];
+        T2 z; z.x = (T)0; z.y = (T)0;
+        x[i] = z;
+        r[i] = b;
+        acc += (double)b.x * (double)b.x + (double)b.y * (double)b.y;
+    }
+    double s = block_sum(acc, red);
+    if (threadIdx.x == 0) part_rr[blockIdx.x] = s;
+}
+
+// alpha = <r,z> / <d,Od>;  x += alpha d;  r -= alpha Od;  part_rr = partial ||r||^2
+template <typename T>
+__global__ void k_cg_axpy(size_t N, typename Cx<T>::type *__restrict__ x, typename Cx<T>::type *__restrict__ r,
+                          const typename Cx<T>::type *__restrict__ d, const typename Cx<T>::type *__restrict__ Od,
+                          const double *__restrict__ part_rz, int n_rz, const double *__restrict__ part_dOd, int n_dOd,
+                          double *__restrict__ part_rr, const CgState *__restrict__ st) {
+    typedef typename Cx<T>::type T2;
+    if (*(volatile const int *)&st->done) return;
+    __shared__ double red[32];
+    __shared__ double s_alpha;
+    double rz = sum_partials_warp0(part_rz, n_rz);
+    double dOd = sum_partials_warp0(part_dOd, n_dOd);
+    if (threadIdx.x == 0) s_alpha = rz / dOd;
+    __syncthreads();
+    const T alpha = (T)s_alpha;
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        T2 xi = x[i], ri = r[i], di = d[i], oi = Od[i];
+        xi.x = fma(alpha, di.x, xi.x); xi.y = fma(alpha, di.y, xi.y);
+        ri.x = fma(-alpha, oi.x, ri.x); ri.y = fma(-alpha, oi.y, ri.y);
+        x[i] = xi; r[i] = ri;
+        acc += (double)ri.x * (double)ri.x + (double)ri.y * (double)ri.y;
+    }
+    double s = block_sum(acc, red);
+    if (threadIdx.x == 0) part_rr[blockIdx.x] = s;
+}
+
+// z = P r (banded in tau, site diagonal, antiperiodic wrap), part_rz = partial Re<r,z>.
+// mode 0: plain apply (no bookkeeping, st may be NULL);  mode 1: CG start (bb = sum part_rr, iters = 0);
+// mode 2: CG iteration (rr = sum part_rr, ++iters, convergence / fixed-count test -> done).
+// Thread i handles spatial site s = i mod Vs for one slice: loads are coalesced along s and the 2W
+// neighbouring slices are re-read from L1/L2 (the halo is on-chip reuse, not algorithmic traffic).
+template <typename T>
+__global__ void k_precond(Geo g, Taps taps, const typename Cx<T>::type *__restrict__ r, typename Cx<T>::type *__restrict__ z,
+                          double *__restrict__ part_rz, const double *__restrict__ part_rr, int n_rr, CgState *st, int mode) {
+    typedef typename Cx<T>::type T2;
+    if (mode != 0 && *(volatile const int *)&st->done) return;
+    __shared__ double red[32];
+    const size_t N = (size_t)g.Vs * g.Nt;
+    const int W = taps.W, Nt = g.Nt;
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        int t = (int)(i / (size_t)g.Vs);
+        size_t s = i - (size_t)t * g.Vs;
+        T2 ri = r[i];
+        double zx = taps.p[0] * (double)ri.x, zy = taps.p[0] * (double)ri.y;
+        for (int m = 1; m <= W; ++m) {
+            int ta = t + m, tb = t - m;
+            double sa = 1.0, sb = 1.0;
+            if (ta >= Nt) { ta -= Nt; sa = -1.0; }
+            if (tb < 0) { tb += Nt; sb = -1.0; }
+            T2 a = r[(size_t)ta * g.Vs + s], b = r[(size_t)tb * g.Vs + s];
+            double pm = taps.p[m];
+            zx = fma(pm, sa * (double)a.x + sb * (double)b.x, zx);
+            zy = fma(pm, sa * (double)a.y + sb * (double)b.y, zy);
+        }
+        T2 zi; zi.x = (T)zx; zi.y = (T)zy;
+        z[i] = zi;
+        acc += (double)ri.x * (double)zi.x + (double)ri.y * (double)zi.y;
+    }
+    double sblk = block_sum(acc, red);
+    if (threadIdx.x == 0 && part_rz != nullptr) part_rz[blockIdx.x] = sblk;
+    if (mode != 0 && blockIdx.x == 0) {
+        double rr = sum_partials_warp0(part_rr, n_rr);
+        if (threadIdx.x == 0) {
+            if (mode == 1) {
+                st->bb = rr; st->rr = rr; st->iters = 0;
+                st->done = (rr == 0.0 || st->max_iter <= 0) ? 1 : 0;
+            } else {
+                long long it = st->iters + 1;
+                st->iters = it; st->rr = rr;
+                if ((st->tol2 > 0.0 && rr <= st->tol2 * st->bb) || it >= st->max_iter) st->done = 1;
+            }
+        }
+    }
+}
+
+// beta = <r,z>_new / <r,z>_old;  d = z + beta d   (first: d = z)
+template <typename T>
+__global__ void k_cg_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, const typename Cx<T>::type *__restrict__ z,
+                             const double *__restrict__ part_new, const double *__restrict__ part_old, int n,
+                             int first, const CgState *__restrict__ st) {
+    typedef typename Cx<T>::type T2;
+    if (*(volatile const int *)&st->done) return;
+    __shared__ double s_beta;
+    if (first) {
+        if (threadIdx.x == 0) s_beta = 0.0;
+    } else {
+        double a = sum_partials_warp0(part_new, n);
+        double b = sum_partials_warp0(part_old, n);
+        if (threadIdx.x == 0) s_beta = a / b;
+    }
+    __syncthreads();
+    const T beta = (T)s_beta;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        T2 zi = z[i];
+        if (!first) { T2 di = d[i]; zi.x = fma(beta, di.x, zi.x); zi.y = fma(beta, di.y, zi.y); }
+        d[i] = zi;
+    }
+}
+
+// Generic deterministic reductions for the energies (Eq.12).
+// kind 0: sum p^2 over doubles a[0..n);  kind 1: Re <a, b> over complex vectors of n elements.
+template <typename T>
+__global__ void k_reduce(int kind, size_t n, const void *__restrict__ a_, const void *__restrict__ b_, double *__restrict__ part) {
+    typedef typename Cx<T>::type T2;
+    __shared__ double red[32];
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        if (kind == 0) { double v = ((const double *)a_)[i]; acc = fma(v, v, acc); }
+        else { T2 a = ((const T2 *)a_)[i], b = ((const T2 *)b_)[i]; acc += (double)a.x * (double)b.x + (double)a.y * (double)b.y; }
+    }
+    double s = block_sum(acc, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = s;
+}
+
+// out[slot] = sum of n partials (single CTA, fixed order)
+__global__ void k_final_sum(const double *__restrict__ part, int n, double *__restrict__ out) {
+    double s = sum_partials_warp0(part, n);
+    if (threadIdx.x == 0) *out = s;
+}
+
+}  // namespace hqmc

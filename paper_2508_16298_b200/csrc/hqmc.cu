@@ -1,0 +1,151 @@
+// hqmc.cu -- C ABI of libhqmc.so (host orchestration).  See include/hqmc.h.
+#include "hqmc_ctx.h"
+
+#include <type_traits>
+
+namespace hqmc {
+
+thread_local std::string g_last_error;
+
+// ---------------------------------------------------------------------------------------------------
+// instrumentation + launch wrapper
+// ---------------------------------------------------------------------------------------------------
+static int drain_events(hqmc_ctx *c) {
+    for (auto &ep : c->pending) {
+        CUDA_TRY(cudaEventSynchronize(ep.b));
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, ep.a, ep.b));
+        c->ms[ep.kclass] += (double)ms;
+        c->pool.push_back(ep);
+    }
+    c->pending.clear();
+    return HQMC_OK;
+}
+
+template <typename... KArgs, typename... Args>
+static int launch(hqmc_ctx *c, int kclass, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args) {
+    if (c->capturing) c->graph_nodes[kclass]++; else c->launches[kclass]++;
+    const bool prof = c->profiling && !c->capturing;
+    EventPair ep{};
+    if (prof) {
+        if (c->pending.size() >= 2048) HQ_TRY(drain_events(c));
+        if (!c->pool.empty()) { ep = c->pool.back(); c->pool.pop_back(); }
+        else { CUDA_TRY(cudaEventCreate(&ep.a)); CUDA_TRY(cudaEventCreate(&ep.b)); }
+        ep.kclass = kclass;
+        CUDA_TRY(cudaEventRecord(ep.a, c->stream));
+    }
+    kernel<<<grid, block, smem, c->stream>>>(static_cast<KArgs>(args)...);
+    CUDA_TRY(cudaGetLastError());
+    if (prof) { CUDA_TRY(cudaEventRecord(ep.b, c->stream)); c->pending.push_back(ep); }
+    return HQMC_OK;
+}
+
+// Dispatch on (BPT, MAXT): f(integral_constant<int,BPT>, integral_constant<int,MAXT>)
+template <typename F> static int with_cfg(const hqmc_ctx *c, F &&f) {
+    using std::integral_constant;
+    if (c->cfg.bpt == 1 && c->cfg.maxt == 256) return f(integral_constant<int, 1>(), integral_constant<int, 256>());
+    if (c->cfg.bpt == 1 && c->cfg.maxt == 576) return f(integral_constant<int, 1>(), integral_constant<int, 576>());
+    if (c->cfg.bpt == 2 && c->cfg.maxt == 576) return f(integral_constant<int, 2>(), integral_constant<int, 576>());
+    if (c->cfg.bpt == 4 && c->cfg.maxt == 576) return f(integral_constant<int, 4>(), integral_constant<int, 576>());
+    g_last_error = "unsupported kernel configuration";
+    return HQMC_EINVAL;
+}
+
+static size_t block_smem(const hqmc_ctx *c) { return (size_t)4 * c->g.nb * c->esz + 32 * sizeof(double); }
+
+template <typename T> static int set_attrs(hqmc_ctx *c) {
+    const int smem = (int)block_smem(c);
+    return with_cfg(c, [&](auto bpt, auto maxt) -> int {
+        constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
+        const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+        CUDA_TRY(cudaFuncSetAttribute(k_apply_M<T, B, M>, attr, smem));
+        CUDA_TRY(cudaFuncSetAttribute(k_apply_B<T, B, M>, attr, smem));
+        CUDA_TRY(cudaFuncSetAttribute(k_mdagm<T, B, M, false>, attr, smem));
+        CUDA_TRY(cudaFuncSetAttribute(k_mdagm<T, B, M, true>, attr, smem));
+        CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, false>, attr, smem));
+        CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, true>, attr, smem));
+        return HQMC_OK;
+    });
+}
+
+template <typename T> static int auto_time_tile(hqmc_ctx *c) {
+    int per_sm = 1;
+    int s = with_cfg(c, [&](auto bpt, auto maxt) -> int {
+        constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_mdagm<T, B, M, true>, c->cfg.threads, block_smem(c)));
+        return HQMC_OK;
+    });
+    if (s != HQMC_OK) return s;
+    if (per_sm < 1) per_sm = 1;
+    int slots = per_sm * c->n_sm;
+    int tt = (c->g.Nt + slots - 1) / slots;
+    c->time_tile = tt < 1 ? 1 : tt;
+    return HQMC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// typed operation launchers
+// ---------------------------------------------------------------------------------------------------
+template <typename T> static int do_phase(hqmc_ctx *c, const double *p, double two_eps) {
+    typedef typename Cx<T>::type T2;
+    if (p) return launch(c, HQMC_K_PHASE, k_phase<T, true>, dim3(c->grid_ew), dim3(256), 0, c->g, c->d_theta, p, two_eps,
+                         (T2 *)c->d_ph, c->th_full, c->th_half);
+    return launch(c, HQMC_K_PHASE, k_phase<T, false>, dim3(c->grid_ew), dim3(256), 0, c->g, c->d_theta, (const double *)nullptr,
+                  0.0, (T2 *)c->d_ph, c->th_full, c->th_half);
+}
+
+template <typename T> static int do_apply_M(hqmc_ctx *c, const void *in, void *out, int dagger) {
+    typedef typename Cx<T>::type T2;
+    return with_cfg(c, [&](auto bpt, auto maxt) -> int {
+        constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
+        return launch(c, HQMC_K_M, k_apply_M<T, B, M>, dim3(c->g.Nt), dim3(c->cfg.threads), block_smem(c), c->g,
+                      (const T2 *)c->d_ph, (const T2 *)in, (T2 *)out, dagger, (T)c->C);
+    });
+}
+
+template <typename T> static int do_mdagm(hqmc_ctx *c, const void *in, void *out, bool dot, const CgState *st) {
+    typedef typename Cx<T>::type T2;
+    const int Tt = c->time_tile;
+    const int grid = (c->g.Nt + Tt - 1) / Tt;
+    c->grid_mdagm = grid;
+    return with_cfg(c, [&](auto bpt, auto maxt) -> int {
+        constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
+        if (dot)
+            return launch(c, HQMC_K_MDAGM, k_mdagm<T, B, M, true>, dim3(grid), dim3(c->cfg.threads), block_smem(c), c->g, Tt,
+                          (const T2 *)c->d_ph, (const T2 *)in, (T2 *)out, (T)c->C, c->d_part_dOd, st);
+        return launch(c, HQMC_K_MDAGM, k_mdagm<T, B, M, false>, dim3(grid), dim3(c->cfg.threads), block_smem(c), c->g, Tt,
+                      (const T2 *)c->d_ph, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st);
+    });
+}
+
+template <typename T> static int do_precond(hqmc_ctx *c, const void *in, void *out, double *part_rz, int mode) {
+    typedef typename Cx<T>::type T2;
+    return launch(c, HQMC_K_PRECOND, k_precond<T>, dim3(c->grid_ew), dim3(256), 0, c->g, c->taps, (const T2 *)in, (T2 *)out,
+                  part_rz, (const double *)c->d_part_rr, c->grid_ew, c->d_state, mode);
+}
+
+template <typename T> static int do_force(hqmc_ctx *c, const void *X, double *out, bool fuse_p, double half_eps, int nkick) {
+    typedef typename Cx<T>::type T2;
+    return with_cfg(c, [&](auto bpt, auto maxt) -> int {
+        constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
+        if (fuse_p)
+            return launch(c, HQMC_K_FORCE, k_force<T, B, M, true>, dim3(c->g.Nt), dim3(c->cfg.threads), block_smem(c), c->g,
+                          (const T2 *)c->d_ph, (const T2 *)X, (T)c->C, out, (const double *)c->d_theta, half_eps,
+                          c->prm.c_tau, c->prm.K, c->prm.compact, nkick);
+        return launch(c, HQMC_K_FORCE, k_force<T, B, M, false>, dim3(c->g.Nt), dim3(c->cfg.threads), block_smem(c), c->g,
+                      (const T2 *)c->d_ph, (const T2 *)X, (T)c->C, out, (const double *)c->d_theta, 0.0, c->prm.c_tau,
+                      c->prm.K, c->prm.compact, 0);
+    });
+}
+
+#define DISPATCH_T(c, call_d, call_f) ((c)->prm.prec == HQMC_C128 ? (call_d) : (call_f))
+
+static bool aligned16(const void *p) { return p != nullptr && (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace hqmc
+
+using namespace hqmc;
+
+#include "hqmc_api_setup.inl"
+#include "hqmc_api_cg.inl"
+#include "hqmc_api_md.inl"

@@ -1,0 +1,92 @@
+// hqmc_api_cg.inl -- preconditioned CG driver (Eq.20; readings C8, C9).
+//
+// One iteration = 4 kernels: [O d + <d,Od>] [x,r update + ||r||^2] [z = P r + <r,z> + bookkeeping]
+// [d = z + beta d].  All scalars (alpha, beta, convergence flag, iteration count) live on the device,
+// so a chunk of iterations is captured ONCE in a CUDA graph and replayed; unlike the
+// paper's fixed-count graph every kernel tests the device-side `done` flag and turns
+// into a no-op after convergence, so tolerance-based stopping and graph replay coexist.  The host looks
+// at the flag once per chunk.
+
+template <typename T> static int cg_iteration(hqmc_ctx *c, void *x, int par) {
+    typedef typename Cx<T>::type T2;
+    HQ_TRY(do_mdagm<T>(c, c->d_d, c->d_Od, true, c->d_state));
+    HQ_TRY(launch(c, HQMC_K_AXPY, k_cg_axpy<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_r, (const T2 *)c->d_d,
+                  (const T2 *)c->d_Od, (const double *)c->d_part_rz[par], c->grid_ew, (const double *)c->d_part_dOd,
+                  c->grid_mdagm, c->d_part_rr, (const CgState *)c->d_state));
+    HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[par ^ 1], 2));
+    HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)c->d_z,
+                  (const double *)c->d_part_rz[par ^ 1], (const double *)c->d_part_rz[par], c->grid_ew, 0,
+                  (const CgState *)c->d_state));
+    return HQMC_OK;
+}
+
+template <typename T> static int cg_build_graph(hqmc_ctx *c, void *x) {
+    if (c->cg_graph && c->cg_graph_x == x && c->cg_graph_tile == c->time_tile) return HQMC_OK;
+    if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+    for (int i = 0; i < HQMC_K_COUNT; ++i) c->graph_nodes[i] = 0;
+    cudaGraph_t graph = nullptr;
+    CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+    c->capturing = true;
+    int st = HQMC_OK;
+    for (int i = 0; i < c->cg_chunk && st == HQMC_OK; ++i) st = cg_iteration<T>(c, x, i & 1);
+    c->capturing = false;
+    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (st != HQMC_OK) { if (graph) cudaGraphDestroy(graph); return st; }
+    CUDA_TRY(e);
+    e = cudaGraphInstantiate(&c->cg_graph, graph, 0);
+    cudaGraphDestroy(graph);
+    CUDA_TRY(e);
+    c->cg_graph_x = x;
+    c->cg_graph_tile = c->time_tile;
+    return HQMC_OK;
+}
+
+template <typename T> static int cg_solve_t(hqmc_ctx *c, const void *rhs, void *x, double tol, long long max_iter,
+                                            long long *iters_out, double *relres_out) {
+    typedef typename Cx<T>::type T2;
+    // state
+    c->h_state->bb = 0.0; c->h_state->rr = 0.0; c->h_state->tol2 = tol > 0.0 ? tol * tol : 0.0;
+    c->h_state->iters = 0; c->h_state->max_iter = max_iter; c->h_state->done = 0; c->h_state->pad = 0;
+    CUDA_TRY(cudaMemcpyAsync(c->d_state, c->h_state, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
+    // x_0 = 0, r_0 = rhs, z_0 = P r_0, d_0 = z_0
+    HQ_TRY(launch(c, HQMC_K_MISC, k_cg_init<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (const T2 *)rhs, (T2 *)x, (T2 *)c->d_r,
+                  c->d_part_rr));
+    HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[0], 1));
+    HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)c->d_z,
+                  (const double *)c->d_part_rz[0], (const double *)c->d_part_rz[0], c->grid_ew, 1, (const CgState *)c->d_state));
+    const bool use_graph = !c->profiling;
+    if (use_graph) HQ_TRY(cg_build_graph<T>(c, x));
+    long long launched = 0;
+    while (true) {
+        if (use_graph) {
+            CUDA_TRY(cudaGraphLaunch(c->cg_graph, c->stream));
+            for (int i = 0; i < HQMC_K_COUNT; ++i) c->launches[i] += c->graph_nodes[i];
+        } else {
+            for (int i = 0; i < c->cg_chunk; ++i) HQ_TRY(cg_iteration<T>(c, x, i & 1));
+        }
+        launched += c->cg_chunk;
+        CUDA_TRY(cudaMemcpyAsync(c->h_state, c->d_state, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(cudaStreamSynchronize(c->stream));
+        if (c->h_state->done) break;
+        if (launched > max_iter + c->cg_chunk) { g_last_error = "CG bookkeeping failed to terminate"; return HQMC_ECUDA; }
+    }
+    const double bb = c->h_state->bb, rr = c->h_state->rr;
+    const double rel = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
+    if (iters_out) *iters_out = c->h_state->iters;
+    if (relres_out) *relres_out = rel;
+    if (tol > 0.0 && rel > tol) return HQMC_ENOCONV;
+    return HQMC_OK;
+}
+
+static int cg_solve_any(hqmc_ctx *c, const void *rhs, void *x, double tol, long long max_iter, long long *iters_out,
+                        double *relres_out) {
+    return DISPATCH_T(c, cg_solve_t<double>(c, rhs, x, tol, max_iter, iters_out, relres_out),
+                      cg_solve_t<float>(c, rhs, x, tol, max_iter, iters_out, relres_out));
+}
+
+extern "C" int hqmc_cg_solve(hqmc_ctx *c, const void *d_rhs, void *d_x, double tol, long long max_iter, long long *iters_out,
+                             double *relres_out) {
+    HQ_TRY(check_vec(c, d_rhs, d_x));
+    if (max_iter < 0) return HQMC_EINVAL;
+    return cg_solve_any(c, d_rhs, d_x, tol, max_iter, iters_out, relres_out);
+}

@@ -1,0 +1,133 @@
+// hqmc_api_md.inl -- forces, energies, leapfrog trajectory (Eq.12, 207-214 Eq.16) and the
+// host-buffer entry points.
+
+extern "C" int hqmc_force(hqmc_ctx *c, const void *d_x, double *d_out) {
+    if (!c || !aligned16(d_x) || !aligned16(d_out)) return HQMC_EINVAL;
+    if (!c->theta_set) { g_last_error = "hqmc_set_theta has not been called"; return HQMC_EINVAL; }
+    return DISPATCH_T(c, do_force<double>(c, d_x, d_out, false, 0.0, 0), do_force<float>(c, d_x, d_out, false, 0.0, 0));
+}
+
+extern "C" int hqmc_force_boson(hqmc_ctx *c, double *d_out) {
+    if (!c || !aligned16(d_out)) return HQMC_EINVAL;
+    if (!c->theta_set) { g_last_error = "hqmc_set_theta has not been called"; return HQMC_EINVAL; }
+    return launch(c, HQMC_K_MISC, k_force_boson, dim3(c->grid_ew), dim3(256), 0, c->g, (const double *)c->d_theta, d_out,
+                  c->prm.c_tau, c->prm.K, c->prm.compact);
+}
+
+// enqueue the reductions; results land in c->d_scal[0..2] = S_B, sum p^2, S_F
+static int enqueue_energies(hqmc_ctx *c, const double *d_p, const void *d_phi, const void *d_x, int slot0) {
+    HQ_TRY(launch(c, HQMC_K_MISC, k_action_boson, dim3(c->grid_ew), dim3(256), 0, c->g, (const double *)c->d_theta, c->prm.c_tau,
+                  c->prm.K, c->prm.compact, c->d_part_misc));
+    HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew, c->d_scal + slot0));
+    if (d_p) {
+        HQ_TRY(launch(c, HQMC_K_MISC, k_reduce<double>, dim3(c->grid_ew), dim3(256), 0, 0, (size_t)2 * c->N, (const void *)d_p,
+                      (const void *)nullptr, c->d_part_misc));
+        HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew,
+                      c->d_scal + slot0 + 1));
+    }
+    if (d_phi && d_x) {
+        if (c->prm.prec == HQMC_C128)
+            HQ_TRY(launch(c, HQMC_K_MISC, k_reduce<double>, dim3(c->grid_ew), dim3(256), 0, 1, c->N, d_phi, d_x, c->d_part_misc));
+        else
+            HQ_TRY(launch(c, HQMC_K_MISC, k_reduce<float>, dim3(c->grid_ew), dim3(256), 0, 1, c->N, d_phi, d_x, c->d_part_misc));
+        HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew,
+                      c->d_scal + slot0 + 2));
+    }
+    return HQMC_OK;
+}
+
+extern "C" int hqmc_energies(hqmc_ctx *c, const double *d_p, const void *d_phi, const void *d_x, double *SB, double *p2, double *SF) {
+    if (!c) return HQMC_EINVAL;
+    if (!c->theta_set) { g_last_error = "hqmc_set_theta has not been called"; return HQMC_EINVAL; }
+    CUDA_TRY(cudaMemsetAsync(c->d_scal, 0, sizeof(double) * 8, c->stream));
+    HQ_TRY(enqueue_energies(c, d_p, d_phi, d_x, 0));
+    CUDA_TRY(cudaMemcpyAsync(c->h_scal, c->d_scal, sizeof(double) * 8, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    if (SB) *SB = c->h_scal[0];
+    if (p2) *p2 = c->h_scal[1];
+    if (SF) *SF = c->h_scal[2];
+    return HQMC_OK;
+}
+
+static int kick(hqmc_ctx *c, double *d_p, double half_eps, int nkick) {
+    return DISPATCH_T(c, do_force<double>(c, c->d_X, d_p, true, half_eps, nkick), do_force<float>(c, c->d_X, d_p, true, half_eps, nkick));
+}
+
+extern "C" int hqmc_leapfrog_trajectory(hqmc_ctx *c, double *d_theta, double *d_p, const void *d_pf, int nsteps, double eps,
+                                        double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
+                                        long long *cg_iters_out) {
+    if (!c || !aligned16(d_theta) || !aligned16(d_p) || !aligned16(d_pf) || nsteps < 0 || cg_max_iter < 0) return HQMC_EINVAL;
+    long long total = 0, it = 0;
+    bool noconv = false;
+    auto solve = [&]() -> int {
+        int s = cg_solve_any(c, d_pf, c->d_X, cg_tol, cg_max_iter, &it, nullptr);
+        total += it;
+        if (s == HQMC_ENOCONV) { noconv = true; return HQMC_OK; }
+        return s;
+    };
+    HQ_TRY(hqmc_set_theta(c, d_theta));
+    CUDA_TRY(cudaMemsetAsync(c->d_scal, 0, sizeof(double) * 8, c->stream));
+    HQ_TRY(solve());
+    HQ_TRY(enqueue_energies(c, d_p, d_pf, c->d_X, 0));                      // H0 parts -> d_scal[0..2]
+    for (int n = 0; n < nsteps; ++n) {
+        if (n == 0) HQ_TRY(kick(c, d_p, 0.5 * eps, 1));                     // p += F(theta_0) eps/2
+        HQ_TRY(DISPATCH_T(c, do_phase<double>(c, d_p, 2.0 * eps), do_phase<float>(c, d_p, 2.0 * eps)));   // theta += 2 p eps
+        HQ_TRY(solve());
+        HQ_TRY(kick(c, d_p, 0.5 * eps, (n == nsteps - 1) ? 1 : 2));         // closing half kick (+ opening one of step n+1)
+    }
+    HQ_TRY(enqueue_energies(c, d_p, d_pf, c->d_X, 3));                      // H1 parts -> d_scal[3..5]
+    if (d_theta != c->d_theta)
+        CUDA_TRY(cudaMemcpyAsync(d_theta, c->d_theta, sizeof(double) * 2 * c->N, cudaMemcpyDeviceToDevice, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->h_scal, c->d_scal, sizeof(double) * 8, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    if (H0_out) *H0_out = c->h_scal[0] + c->h_scal[1] + c->h_scal[2];
+    if (H1_out) *H1_out = c->h_scal[3] + c->h_scal[4] + c->h_scal[5];
+    if (cg_iters_out) *cg_iters_out = total;
+    return noconv ? HQMC_ENOCONV : HQMC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// host-buffer variants: H2D copies, compute, D2H copies, all on the context's stream
+// ---------------------------------------------------------------------------------------------------
+extern "C" int hqmc_apply_MdagM_host(hqmc_ctx *c, const void *h_in, void *h_out) {
+    if (!c || !h_in || !h_out) return HQMC_EINVAL;
+    const size_t vb = c->N * c->esz;
+    CUDA_TRY(cudaMemcpyAsync(c->d_d, h_in, vb, cudaMemcpyHostToDevice, c->stream));
+    HQ_TRY(hqmc_apply_MdagM(c, c->d_d, c->d_Od));
+    CUDA_TRY(cudaMemcpyAsync(h_out, c->d_Od, vb, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return HQMC_OK;
+}
+
+extern "C" int hqmc_cg_solve_host(hqmc_ctx *c, const double *h_theta, const void *h_rhs, void *h_x, double tol,
+                                  long long max_iter, long long *iters_out, double *relres_out) {
+    if (!c || !h_rhs || !h_x || max_iter < 0) return HQMC_EINVAL;
+    const size_t vb = c->N * c->esz;
+    if (h_theta) {
+        CUDA_TRY(cudaMemcpyAsync(c->d_theta, h_theta, sizeof(double) * 2 * c->N, cudaMemcpyHostToDevice, c->stream));
+        HQ_TRY(hqmc_set_theta(c, c->d_theta));
+    }
+    if (!c->theta_set) { g_last_error = "no theta"; return HQMC_EINVAL; }
+    CUDA_TRY(cudaMemcpyAsync(c->d_phi, h_rhs, vb, cudaMemcpyHostToDevice, c->stream));
+    int s = cg_solve_any(c, c->d_phi, c->d_X, tol, max_iter, iters_out, relres_out);
+    if (s != HQMC_OK && s != HQMC_ENOCONV) return s;
+    CUDA_TRY(cudaMemcpyAsync(h_x, c->d_X, vb, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return s;
+}
+
+extern "C" int hqmc_leapfrog_trajectory_host(hqmc_ctx *c, double *h_theta, double *h_p, const void *h_pf, int nsteps, double eps,
+                                             double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
+                                             long long *cg_iters_out) {
+    if (!c || !h_theta || !h_p || !h_pf) return HQMC_EINVAL;
+    const size_t vb = c->N * c->esz, tb = sizeof(double) * 2 * c->N;
+    CUDA_TRY(cudaMemcpyAsync(c->d_theta, h_theta, tb, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->d_p, h_p, tb, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->d_phi, h_pf, vb, cudaMemcpyHostToDevice, c->stream));
+    int s = hqmc_leapfrog_trajectory(c, c->d_theta, c->d_p, c->d_phi, nsteps, eps, cg_tol, cg_max_iter, H0_out, H1_out, cg_iters_out);
+    if (s != HQMC_OK && s != HQMC_ENOCONV) return s;
+    CUDA_TRY(cudaMemcpyAsync(h_theta, c->d_theta, tb, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(h_p, c->d_p, tb, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return s;
+}

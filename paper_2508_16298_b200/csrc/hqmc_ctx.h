@@ -1,0 +1,80 @@
+// hqmc_ctx.h -- private context of libhqmc.so and launch helpers (host code).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/hqmc.h"
+#include "cg_kernels.cuh"
+#include "force_kernels.cuh"
+#include "kernels.cuh"
+
+namespace hqmc {
+
+extern thread_local std::string g_last_error;
+
+#define CUDA_TRY(expr)                                                                                     \
+    do {                                                                                                   \
+        cudaError_t _e = (expr);                                                                           \
+        if (_e != cudaSuccess) {                                                                           \
+            g_last_error = std::string(#expr) + ": " + cudaGetErrorString(_e);                             \
+            return (_e == cudaErrorMemoryAllocation) ? HQMC_ENOMEM : HQMC_ECUDA;                           \
+        }                                                                                                  \
+    } while (0)
+#define HQ_TRY(expr)                                                                                       \
+    do {                                                                                                   \
+        int _s = (expr);                                                                                   \
+        if (_s != HQMC_OK) return _s;                                                                      \
+    } while (0)
+
+struct KernelCfg { int bpt; int maxt; int threads; };
+
+struct EventPair { cudaEvent_t a, b; int kclass; };
+
+}  // namespace hqmc
+
+struct hqmc_ctx {
+    hqmc_params prm;
+    hqmc::Geo g;
+    size_t N;            // sites
+    size_t esz;          // bytes per complex element
+    cudaStream_t stream;
+    bool own_stream;
+    int n_sm;
+    hqmc::KernelCfg cfg;
+    int time_tile;       // slices per CTA of k_mdagm (0 = auto)
+    double C;            // cosh(a/2)^6 cosh(a)
+    double th_full, th_half;
+    hqmc::Taps taps;
+    // device memory owned by the context
+    double *d_theta;     // copy of the gauge field
+    void *d_ph;          // phase table [Nt][2][L][L] complex
+    void *d_r, *d_z, *d_d, *d_Od, *d_X, *d_phi;   // CG vectors, trajectory solution / pseudofermion
+    double *d_p, *d_force;                        // host-variant staging
+    double *d_part_dOd, *d_part_rr, *d_part_rz[2], *d_part_misc;
+    hqmc::CgState *d_state;
+    hqmc::CgState *h_state;  // pinned
+    double *d_scal;          // 8 doubles
+    double *h_scal;          // pinned
+    bool theta_set;
+    // grids
+    int grid_ew, grid_mdagm;
+    // CG chunk graph
+    cudaGraphExec_t cg_graph;
+    void *cg_graph_x;        // x pointer baked into the graph
+    int cg_graph_tile;
+    int cg_chunk;            // iterations per graph launch
+    // instrumentation
+    bool profiling;
+    bool capturing;
+    long long launches[HQMC_K_COUNT];
+    long long graph_nodes[HQMC_K_COUNT];   // kernels of each class inside one cg_graph replay
+    double ms[HQMC_K_COUNT];
+    std::vector<hqmc::EventPair> pending;
+    std::vector<hqmc::EventPair> pool;
+};

@@ -1,0 +1,215 @@
+"""Thin ctypes binding of libhqmc.so (include/hqmc.h).  Argument marshalling only: every step of the
+hot path runs in the library's CUDA kernels.  PyTorch is used for device memory and streams.
+
+There is NO CPU fallback: importing this module raises if libhqmc.so is missing, and every compute
+call raises HqmcError if the library reports an error (e.g. no CUDA device).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhqmc.so")
+
+HQMC_OK, HQMC_EINVAL, HQMC_ECUDA, HQMC_ENOCONV, HQMC_ENOMEM = 0, -1, -2, -3, -4
+K_MDAGM, K_AXPY, K_PRECOND, K_DUPDATE, K_M, K_FORCE, K_PHASE, K_MISC, K_COUNT = range(9)
+KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force", "phase", "misc"]
+
+# every symbol include/hqmc.h declares
+SYMBOLS = [
+    "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
+    "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_apply_MdagM_host", "hqmc_cg_solve_host",
+    "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
+    "hqmc_set_time_tile", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
+]
+
+
+class HqmcError(RuntimeError):
+    pass
+
+
+class _Params(C.Structure):
+    _fields_ = [("L", C.c_int), ("Ntau", C.c_int), ("dtau", C.c_double), ("t", C.c_double), ("c_tau", C.c_double),
+                ("K", C.c_double), ("compact", C.c_int), ("precond_W", C.c_int), ("prec", C.c_int)]
+
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2508_16298_b200.build` "
+                      "(there is no CPU fallback)")
+_lib = C.CDLL(LIB_PATH)
+_lib.hqmc_strerror.restype = C.c_char_p
+_lib.hqmc_last_error.restype = C.c_char_p
+for _s in SYMBOLS:
+    getattr(_lib, _s)  # raises AttributeError if a declared symbol is not exported
+
+
+def _check(status: int, allow_noconv: bool = False) -> int:
+    if status == HQMC_OK or (allow_noconv and status == HQMC_ENOCONV):
+        return status
+    raise HqmcError(f"{_lib.hqmc_strerror(status).decode()} ({status}): {_lib.hqmc_last_error().decode()}")
+
+
+def _ptr(t: torch.Tensor) -> C.c_void_p:
+    return C.c_void_p(t.data_ptr())
+
+
+class HQMC:
+    """One lattice + couplings on one GPU.  Vectors are torch complex tensors [Ntau, L, L] on the device,
+    theta / p / forces are float64 tensors [Ntau, 2, L, L]."""
+
+    def __init__(self, L, Ntau, dtau=0.1, t=1.0, c_tau=1.0, K=1.0, compact=True, W=6, prec="c128", device="cuda:0"):
+        self.L, self.Ntau, self.N = L, Ntau, L * L * Ntau
+        self.device = torch.device(device)
+        self.cdtype = torch.complex128 if prec == "c128" else torch.complex64
+        self.np_cdtype = np.complex128 if prec == "c128" else np.complex64
+        p = _Params(L, Ntau, dtau, t, c_tau, K, int(compact), W, 0 if prec == "c128" else 1)
+        self._ctx = C.c_void_p()
+        if self.device.type == "cuda":
+            torch.cuda.set_device(self.device)
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+        else:
+            stream = 0
+        _check(_lib.hqmc_create(C.byref(p), C.c_void_p(stream), C.byref(self._ctx)))
+
+    def close(self):
+        if self._ctx:
+            _lib.hqmc_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- helpers ------------------------------------------------------------------------------
+    def _vec(self, v):
+        assert v.is_cuda and v.dtype == self.cdtype and v.numel() == self.N and v.is_contiguous()
+        return v
+
+    def _field(self, f):
+        assert f.is_cuda and f.dtype == torch.float64 and f.numel() == 2 * self.N and f.is_contiguous()
+        return f
+
+    def new_vec(self):
+        return torch.empty((self.Ntau, self.L, self.L), dtype=self.cdtype, device=self.device)
+
+    def new_field(self):
+        return torch.empty((self.Ntau, 2, self.L, self.L), dtype=torch.float64, device=self.device)
+
+    # ---- setup --------------------------------------------------------------------------------
+    def set_theta(self, theta):
+        _check(_lib.hqmc_set_theta(self._ctx, _ptr(self._field(theta))))
+
+    def set_precond(self, taps):
+        taps = np.ascontiguousarray(taps, dtype=np.float64)
+        _check(_lib.hqmc_set_precond(self._ctx, C.c_int(len(taps) - 1), taps.ctypes.data_as(C.c_void_p)))
+
+    def get_precond(self):
+        W = C.c_int(0)
+        taps = np.zeros(33)
+        _check(_lib.hqmc_get_precond(self._ctx, C.byref(W), taps.ctypes.data_as(C.c_void_p)))
+        return taps[: W.value + 1].copy()
+
+    def set_time_tile(self, tt: int):
+        _check(_lib.hqmc_set_time_tile(self._ctx, C.c_int(tt)))
+
+    # ---- operators ----------------------------------------------------------------------------
+    def _apply(self, fn, v, out):
+        out = self.new_vec() if out is None else out
+        _check(fn(self._ctx, _ptr(self._vec(v)), _ptr(self._vec(out))))
+        return out
+
+    def apply_M(self, v, out=None):
+        return self._apply(_lib.hqmc_apply_M, v, out)
+
+    def apply_Mdag(self, v, out=None):
+        return self._apply(_lib.hqmc_apply_Mdag, v, out)
+
+    def apply_MdagM(self, v, out=None):
+        return self._apply(_lib.hqmc_apply_MdagM, v, out)
+
+    def precond(self, v, out=None):
+        return self._apply(_lib.hqmc_precond, v, out)
+
+    def cg_solve(self, rhs, tol=1e-10, max_iter=1000000, x=None):
+        """-> (x, iterations, relative recurrence residual, converged)."""
+        x = self.new_vec() if x is None else x
+        it, rel = C.c_longlong(0), C.c_double(0.0)
+        s = _check(_lib.hqmc_cg_solve(self._ctx, _ptr(self._vec(rhs)), _ptr(self._vec(x)), C.c_double(tol),
+                                      C.c_longlong(max_iter), C.byref(it), C.byref(rel)), allow_noconv=True)
+        return x, it.value, rel.value, s == HQMC_OK
+
+    def force(self, x, out=None):
+        out = self.new_field() if out is None else out
+        _check(_lib.hqmc_force(self._ctx, _ptr(self._vec(x)), _ptr(self._field(out))))
+        return out
+
+    def force_boson(self, out=None):
+        out = self.new_field() if out is None else out
+        _check(_lib.hqmc_force_boson(self._ctx, _ptr(self._field(out))))
+        return out
+
+    def energies(self, p=None, phi=None, x=None):
+        """-> (S_B, sum p^2, S_F) at the context's theta."""
+        SB, p2, SF = C.c_double(0), C.c_double(0), C.c_double(0)
+        _check(_lib.hqmc_energies(self._ctx, _ptr(self._field(p)) if p is not None else None,
+                                  _ptr(self._vec(phi)) if phi is not None else None,
+                                  _ptr(self._vec(x)) if x is not None else None, C.byref(SB), C.byref(p2), C.byref(SF)))
+        return SB.value, p2.value, SF.value
+
+    def trajectory(self, theta, p, phi, nsteps, eps, cg_tol=1e-10, cg_max_iter=1000000):
+        """In place on theta, p.  -> dict(H0, H1, cg_iters, converged)."""
+        H0, H1, it = C.c_double(0), C.c_double(0), C.c_longlong(0)
+        s = _check(_lib.hqmc_leapfrog_trajectory(self._ctx, _ptr(self._field(theta)), _ptr(self._field(p)),
+                                                 _ptr(self._vec(phi)), C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol),
+                                                 C.c_longlong(cg_max_iter), C.byref(H0), C.byref(H1), C.byref(it)),
+                   allow_noconv=True)
+        return dict(H0=H0.value, H1=H1.value, cg_iters=it.value, converged=(s == HQMC_OK))
+
+    # ---- host-buffer entry points (numpy arrays, pageable or pinned) ----------------------------
+    def apply_MdagM_host(self, h_in: np.ndarray, h_out: np.ndarray):
+        assert h_in.dtype == self.np_cdtype and h_out.dtype == self.np_cdtype and h_in.size == self.N == h_out.size
+        _check(_lib.hqmc_apply_MdagM_host(self._ctx, h_in.ctypes.data_as(C.c_void_p), h_out.ctypes.data_as(C.c_void_p)))
+        return h_out
+
+    def cg_solve_host(self, h_theta, h_rhs, h_x, tol=1e-10, max_iter=1000000):
+        it, rel = C.c_longlong(0), C.c_double(0.0)
+        th = h_theta.ctypes.data_as(C.c_void_p) if h_theta is not None else None
+        s = _check(_lib.hqmc_cg_solve_host(self._ctx, th, h_rhs.ctypes.data_as(C.c_void_p), h_x.ctypes.data_as(C.c_void_p),
+                                           C.c_double(tol), C.c_longlong(max_iter), C.byref(it), C.byref(rel)), allow_noconv=True)
+        return h_x, it.value, rel.value, s == HQMC_OK
+
+    def trajectory_host(self, h_theta, h_p, h_phi, nsteps, eps, cg_tol=1e-10, cg_max_iter=1000000):
+        H0, H1, it = C.c_double(0), C.c_double(0), C.c_longlong(0)
+        s = _check(_lib.hqmc_leapfrog_trajectory_host(self._ctx, h_theta.ctypes.data_as(C.c_void_p),
+                                                      h_p.ctypes.data_as(C.c_void_p), h_phi.ctypes.data_as(C.c_void_p),
+                                                      C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol),
+                                                      C.c_longlong(cg_max_iter), C.byref(H0), C.byref(H1), C.byref(it)),
+                   allow_noconv=True)
+        return dict(H0=H0.value, H1=H1.value, cg_iters=it.value, converged=(s == HQMC_OK))
+
+    # ---- instrumentation ----------------------------------------------------------------------
+    def set_profiling(self, on: bool):
+        _check(_lib.hqmc_set_profiling(self._ctx, C.c_int(int(on))))
+
+    def reset_stats(self):
+        _check(_lib.hqmc_reset_stats(self._ctx))
+
+    def kernel_stats(self):
+        """-> {class: (launches, summed device ms)}"""
+        out = {}
+        for i, name in enumerate(KERNEL_CLASSES):
+            n, ms = C.c_longlong(0), C.c_double(0)
+            _check(_lib.hqmc_get_kernel_stats(self._ctx, C.c_int(i), C.byref(n), C.byref(ms)))
+            out[name] = (n.value, ms.value)
+        return out
+
+
+def version() -> int:
+    return int(_lib.hqmc_version())

@@ -1,0 +1,179 @@
+"""GPU parity: libhqmc.so (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's north_star: <= 1e-12 relative per M / M^+ application,
+<= 1e-9 per CG solution (tol 1e-10), <= 1e-9 per force component, <= 1e-8 in dH, reversibility <= 1e-10."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2508_16298_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hq(cuda_device):
+    from paper_2508_16298_b200 import hqmc
+    return hqmc
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rel(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def setup(hq, L, Nt, seed, theta=None, **kw):
+    theta = inputs.theta_uniform(L, Nt, seed) if theta is None else theta
+    o = orc.Oracle(L, Nt, **kw)
+    orc.set_threads(orc.max_threads())
+    g = hq.HQMC(L, Nt, **kw)
+    g.set_theta(dev(theta))
+    return o, g, theta
+
+
+# sizes: tiny (config 1), odd-shaped, several warps with ragged thread tail, BPT=2 and BPT=4 code paths
+SHAPES = [(4, 8, 0), (6, 10, 1), (12, 14, 2), (18, 7, 3), (34, 5, 4), (50, 4, 5), (70, 3, 6)]
+
+
+@pytest.mark.parametrize("L,Nt,seed", SHAPES)
+def test_M_Mdag_MdagM(hq, L, Nt, seed):
+    o, g, theta = setup(hq, L, Nt, seed, W=min(6, Nt - 1))
+    v = inputs.complex_gaussian((Nt, L, L), seed, inputs.STREAM_VEC)
+    dv = dev(v)
+    assert rel(g.apply_M(dv).cpu().numpy(), o.apply_M(theta, v)) <= 1e-12
+    assert rel(g.apply_Mdag(dv).cpu().numpy(), o.apply_Mdag(theta, v)) <= 1e-12
+    ref = o.apply_MdagM(theta, v)
+    assert rel(g.apply_MdagM(dv).cpu().numpy(), ref) <= 1e-12
+    for tt in (1, 2, 3, Nt):          # every time-tile shape incl. ragged last tile and one-CTA-for-all
+        g.set_time_tile(tt)
+        assert rel(g.apply_MdagM(dv).cpu().numpy(), ref) <= 1e-12
+    g.close()
+
+
+def test_config2_twenty_MdagM(hq):
+    """BASELINE config 2: L=12, Ntau=120, heat-bath theta, 20 seeded M^+M applications."""
+    c = inputs.CONFIGS[2]
+    theta = inputs.make_theta(2)
+    o, g, _ = setup(hq, c["L"], c["Ntau"], c["seed"], theta=theta)
+    vs = inputs.bench_vectors(20, c["L"], c["Ntau"], c["seed"])
+    worst = 0.0
+    for v in vs:
+        worst = max(worst, rel(g.apply_MdagM(dev(v)).cpu().numpy(), o.apply_MdagM(theta, v)))
+    assert worst <= 1e-12
+    g.close()
+
+
+@pytest.mark.parametrize("L,Nt,W", [(4, 8, 6), (6, 10, 3), (12, 30, 6), (4, 8, 0)])
+def test_precond_and_taps(hq, L, Nt, W):
+    o, g, theta = setup(hq, L, Nt, 3, W=W)
+    if W > 0:
+        assert np.abs(g.get_precond() - o.taps).max() <= 1e-13 * o.taps.max()
+    v = inputs.complex_gaussian((Nt, L, L), 7, inputs.STREAM_VEC)
+    ref = o.precond(v) if W > 0 else v
+    assert rel(g.precond(dev(v)).cpu().numpy(), ref) <= 1e-13
+    g.close()
+
+
+@pytest.mark.parametrize("L,Nt,seed,W", [(4, 8, 0, 6), (4, 8, 0, 0), (6, 10, 1, 6), (8, 40, 2, 6)])
+def test_cg_solution_and_iterations(hq, L, Nt, seed, W):
+    o, g, theta = setup(hq, L, Nt, seed, W=W)
+    eta = inputs.complex_gaussian((Nt, L, L), seed)
+    phi = o.apply_Mdag(theta, eta)
+    x_ref, it_ref, rel_ref = o.pcg(theta, phi, 1e-10, 100000)
+    x, it, relres, ok = g.cg_solve(dev(phi), 1e-10, 100000)
+    x = x.cpu().numpy()
+    assert ok and relres <= 1e-10
+    assert abs(it - it_ref) <= max(2, it_ref // 100)
+    # residual of the GPU solution evaluated with the ORACLE's operator (reading C16 i)
+    res = np.linalg.norm((phi - o.apply_MdagM(theta, x)).ravel()) / np.linalg.norm(phi.ravel())
+    assert res <= 1.05e-10
+    # the GPU and oracle iterates at the same tolerance agree to <= 1e-9 (they stop within a few iterations)
+    assert rel(x, x_ref) <= 1e-9
+    # forward error against an oracle solve converged to 1e-13 (C16 ii): bounded by cond(M^+M) * residual, so
+    # <= 1e-9 at tol 1e-10 only while cond is moderate (config 1: 71); otherwise it is met at a tighter tol.
+    x13 = o.pcg(theta, phi, 1e-13, 100000)[0]
+    if L == 4:
+        assert rel(x, x13) <= 1e-9
+    else:
+        xt, _, _, okt = g.cg_solve(dev(phi), 1e-12, 100000)
+        assert okt and rel(xt.cpu().numpy(), x13) <= 1e-9
+    # fixed-count mode
+    xf, itf, relf, _ = g.cg_solve(dev(phi), 0.0, 11)
+    xo, ito, relo = o.pcg(theta, phi, 0.0, 11)
+    assert itf == ito == 11 and rel(xf.cpu().numpy(), xo) <= 1e-11 and abs(relf - relo) <= 1e-9 * relo
+    g.close()
+
+
+@pytest.mark.parametrize("L,Nt,seed", [(4, 8, 0), (6, 10, 1), (12, 14, 2), (50, 4, 5)])
+@pytest.mark.parametrize("compact", [True, False])
+def test_forces_and_energies(hq, L, Nt, seed, compact):
+    o, g, theta = setup(hq, L, Nt, seed, c_tau=1.3, K=0.7, compact=compact)
+    X = inputs.complex_gaussian((Nt, L, L), seed + 10, inputs.STREAM_VEC)
+    phi = inputs.complex_gaussian((Nt, L, L), seed + 11, inputs.STREAM_VEC)
+    p = inputs.momenta(L, Nt, seed)
+    gF = g.force(dev(X)).cpu().numpy()
+    ref = o.force_fermion(theta, X)
+    assert np.abs(gF - ref).max() <= 1e-9 * max(1.0, np.abs(ref).max())
+    gB = g.force_boson().cpu().numpy()
+    refB = o.force_boson(theta)
+    assert np.abs(gB - refB).max() <= 1e-12 * max(1.0, np.abs(refB).max())
+    SB, p2, SF = g.energies(dev(p), dev(phi), dev(X))
+    assert abs(SB - o.action_boson(theta)) <= 1e-11 * abs(SB) + 1e-11
+    assert abs(p2 - o.sum_p2(p)) <= 1e-12 * p2
+    assert abs(SF - np.vdot(phi, X).real) <= 1e-11 * max(1.0, abs(SF))
+    g.close()
+
+
+@pytest.mark.parametrize("L,Nt,seed,nsteps", [(4, 8, 0, 8), (6, 10, 1, 5)])
+def test_trajectory_dH_and_reversibility(hq, L, Nt, seed, nsteps):
+    o, g, theta = setup(hq, L, Nt, seed)
+    eta = inputs.complex_gaussian((Nt, L, L), seed)
+    phi = o.apply_Mdag(theta, eta)
+    p = inputs.momenta(L, Nt, seed)
+    ref = o.trajectory(theta, p, phi, nsteps, 0.05, cg_tol=1e-13)
+    dth, dp, dphi = dev(theta), dev(p), dev(phi)
+    r = g.trajectory(dth, dp, dphi, nsteps, 0.05, cg_tol=1e-13)
+    assert r["converged"]
+    assert abs(r["H0"] - ref["H0"]) <= 1e-8 and abs(r["H1"] - ref["H1"]) <= 1e-8
+    assert abs((r["H1"] - r["H0"]) - (ref["H1"] - ref["H0"])) <= 1e-8
+    assert np.abs(dth.cpu().numpy() - ref["theta"]).max() <= 1e-10
+    assert np.abs(dp.cpu().numpy() - ref["p"]).max() <= 1e-10
+    # reversibility on the GPU: flip p, integrate back
+    dp.neg_()
+    g.trajectory(dth, dp, dphi, nsteps, 0.05, cg_tol=1e-13)
+    assert np.abs(dth.cpu().numpy() - theta).max() <= 1e-10
+    assert np.abs(dp.cpu().numpy() + p).max() <= 1e-10
+    g.close()
+
+
+def test_complex64_variant(hq):
+    """Reading C19: <= 1e-6 L2-relative per M^+M against the fp64 oracle."""
+    L, Nt = 12, 30
+    theta = inputs.theta_uniform(L, Nt, 8)
+    o = orc.Oracle(L, Nt)
+    g = hq.HQMC(L, Nt, prec="c64")
+    g.set_theta(dev(theta))
+    v = inputs.complex_gaussian((Nt, L, L), 8, inputs.STREAM_VEC)
+    out = g.apply_MdagM(dev(v.astype(np.complex64))).cpu().numpy().astype(np.complex128)
+    ref = o.apply_MdagM(theta, v)
+    assert np.linalg.norm((out - ref).ravel()) / np.linalg.norm(ref.ravel()) <= 1e-6
+    x, it, relres, _ = g.cg_solve(dev(v.astype(np.complex64)), 0.0, 50)
+    xo, _, relo = o.pcg(theta, v, 0.0, 50)
+    assert it == 50 and np.linalg.norm((x.cpu().numpy() - xo).ravel()) / np.linalg.norm(xo.ravel()) <= 1e-3
+    g.close()
+
+
+def test_host_buffer_entry_points(hq):
+    L, Nt = 6, 10
+    o, g, theta = setup(hq, L, Nt, 4)
+    v = inputs.complex_gaussian((Nt, L, L), 4, inputs.STREAM_VEC)
+    out = np.empty_like(v)
+    g.apply_MdagM_host(v, out)
+    assert rel(out, o.apply_MdagM(theta, v)) <= 1e-12
+    x = np.empty_like(v)
+    _, it, relres, ok = g.cg_solve_host(theta, v, x, 1e-10, 10000)
+    assert ok and rel(x, o.pcg(theta, v, 1e-13, 10000)[0]) <= 1e-9
+    g.close()
