@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the HQMC pseudofermion hot path on B200.
+
+A STEP is one pass of the whole hot path on one lattice:
+    phi = M^+(theta) eta                         (S8, pseudofermion refresh)
+    one leapfrog step of the MD trajectory       (S13): 2 fixed-count PCG solves of M^+M x = phi
+        (S5-S7: fused M^+M, preconditioner, fused axpy/dot), force + boson force + momentum kicks
+        (S9, S10), drift + phase table (S11, S1), energies H0, H1 (S12)
+with the paper's fixed-iteration CG protocol: --cg-iters iterations per solve.
+`value` = M^+M applications x sites / time, in Gsite/s (BASELINE.json's metric), for the WHOLE step,
+i.e. it charges the preconditioner, the vector updates, the force and the energies to the M^+M count.
+The other BASELINE quantities ride along in the same JSON line: CG-solve ms (`cg_ms_per_solve`,
+`cg_us_per_iter`), achieved HBM GB/s against the measured peak (`roofline`), ms per trajectory step.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--cg-iters I] [--config 4]
+    python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N ...   (replicas, weak scaling)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "MdagM_Gsite_per_s"
+UNIT = "Gsite/s"
+# algorithmic bytes per site (complex128): read v (16) + 2 link phases as theta (16) + write (16)
+BYTES_PER_SITE = {"mdagm": 48.0, "cg_axpy": 96.0, "precond": 32.0, "cg_dupdate": 48.0}
+BYTES_PER_SITE_C64 = {k: v / 2 for k, v in BYTES_PER_SITE.items()}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# --------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands, on the host cores, on a bounded sample
+# --------------------------------------------------------------------------------------------------
+def oracle_step_sample(L, Ntau, seed, cg_iters, nsteps_md=1, threads=None):
+    """One hot-path step with the CPU oracle (same structure as the GPU step, cg_iters per solve).
+    -> (seconds, MdagM applications, threads used)."""
+    from oracle import oracle as orc
+    from paper_2508_16298_b200 import inputs
+    orc.build()
+    threads = threads or orc.max_threads()
+    orc.set_threads(threads)
+    theta = inputs.theta_uniform(L, Ntau, seed)
+    eta = inputs.complex_gaussian((Ntau, L, L), seed)
+    p = inputs.momenta(L, Ntau, seed)
+    o = orc.Oracle(L, Ntau)
+    t0 = time.perf_counter()
+    phi = o.apply_Mdag(theta, eta)
+    r = o.trajectory(theta, p, phi, nsteps_md, 0.05, cg_tol=0.0, cg_max_iter=cg_iters)
+    dt = time.perf_counter() - t0
+    return dt, r["cg_iters"], orc.get_threads()
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    from paper_2508_16298_b200 import inputs
+    c = inputs.CONFIGS[args.config]
+    L, Ntau, N = c["L"], c["Ntau"], c["L"] * c["L"] * c["Ntau"]
+    iters = args.ref_cg_iters
+    times, apps, threads = [], 0, 1
+    for i in range(args.warmup + args.steps):
+        dt, a, threads = oracle_step_sample(L, Ntau, c["seed"], iters)
+        if i >= args.warmup:
+            times.append(dt); apps += a
+    total = sum(times)
+    value = apps * N / total / 1e9
+    sample = (f"same lattice (L={L}, Ntau={Ntau}), same step structure, fixed-count CG cut to {iters} iterations per solve "
+              f"({2 * iters} M^+M per step) instead of {args.cg_iters}")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / max(1, len(times)), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(args, L, Ntau, iters),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(args, L, Ntau, cg_iters):
+    return {"workload": f"BASELINE config {args.config}: L={L}, Ntau={Ntau}, theta uniform[-pi,pi) (seeded), complex128; "
+                        f"step = M^+ refresh + 1 leapfrog step (2 fixed-count PCG solves, W=6 preconditioner, force, kicks, "
+                        f"drift, energies)",
+            "L": L, "Ntau": Ntau, "sites": L * L * Ntau, "cg_iters_per_solve": cg_iters, "precond_W": 6,
+            "l2": "step footprint (7 fermion vectors + phase table + theta, p) exceeds the 126 MB L2 at L=48; the M^+M "
+                  "kernel sweep additionally rotates 8 input/output buffer pairs"}
+
+
+# --------------------------------------------------------------------------------------------------
+# GPU arm
+# --------------------------------------------------------------------------------------------------
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2508_16298_b200 import hqmc, inputs, replicas
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    c = inputs.CONFIGS[args.config]
+    L, Ntau = c["L"], c["Ntau"]
+    N = L * L * Ntau
+    seed = replicas.replica_seed(c["seed"], rank)          # one independent lattice (Markov chain) per rank
+    prec = args.prec
+    cdt = np.complex128 if prec == "c128" else np.complex64
+    theta0 = inputs.theta_uniform(L, Ntau, seed)
+    eta = inputs.complex_gaussian((Ntau, L, L), seed).astype(cdt)
+    p0 = inputs.momenta(L, Ntau, seed)
+
+    g = hqmc.HQMC(L, Ntau, prec=prec, device=str(dev))
+    to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    d_theta0, d_p0, d_eta = to_dev(theta0), to_dev(p0), to_dev(eta)
+    d_theta, d_p, d_phi = torch.empty_like(d_theta0), torch.empty_like(d_p0), g.new_vec()
+    I = args.cg_iters
+
+    def step_device():
+        d_theta.copy_(d_theta0); d_p.copy_(d_p0)
+        g.set_theta(d_theta)
+        g.apply_Mdag(d_eta, d_phi)
+        return g.trajectory(d_theta, d_p, d_phi, 1, 0.05, cg_tol=0.0, cg_max_iter=I)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        r = step_device()
+    g.reset_stats()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    apps = 0
+    e0.record()
+    for _ in range(args.steps):
+        r = step_device()
+        apps += r["cg_iters"]
+    e1.record()
+    barrier()
+    ms_local = e0.elapsed_time(e1)
+    stats = g.kernel_stats()
+    launches = sum(v[0] for v in stats.values())
+
+    # ---- end to end through the host-buffer entry points (pinned host memory, copies inside the timed region)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_theta0, h_p0, h_eta = pin(theta0), pin(p0), pin(eta)
+    h_theta, h_p, h_phi = torch.empty_like(h_theta0).pin_memory(), torch.empty_like(h_p0).pin_memory(), torch.empty_like(h_eta).pin_memory()
+    n_theta, n_p, n_phi, n_eta = h_theta.numpy(), h_p.numpy(), h_phi.numpy(), h_eta.numpy()
+
+    def step_host():
+        h_theta.copy_(h_theta0); h_p.copy_(h_p0)
+        g.refresh_host(n_theta, n_eta, n_phi)                       # H2D theta, eta; phi = M^+ eta; D2H phi
+        return g.trajectory_host(n_theta, n_p, n_phi, 1, 0.05, cg_tol=0.0, cg_max_iter=I)   # H2D theta, p, phi; D2H theta, p
+
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    step_host()
+    barrier()
+    t0 = time.perf_counter()
+    e2e_apps = 0
+    for _ in range(e2e_steps):
+        e2e_apps += step_host()["cg_iters"]
+    torch.cuda.synchronize()
+    e2e_s_local = time.perf_counter() - t0
+    barrier()
+    vb, tb = N * (16 if prec == "c128" else 8), 2 * N * 8
+    h2d, d2h = (tb + vb) + (2 * tb + vb), vb + 2 * tb
+
+    # ---- per-kernel timing of the same step (library-side CUDA events on the launching stream, no graph replay)
+    kern = None
+    if rank == 0:
+        g.set_profiling(True)
+        step_device(); torch.cuda.synchronize()
+        g.reset_stats()
+        for _ in range(max(1, min(3, args.steps))):
+            step_device()
+        torch.cuda.synchronize()
+        kern = g.kernel_stats()
+        g.set_profiling(False)
+
+    # ---- M^+M kernel alone, cold (rotating 8 buffer pairs > L2) and warm (same buffers)
+    sweep = None
+    if rank == 0 and not args.no_sweep:
+        sweep = mdagm_sweep(g, torch, dev, L, Ntau, prec)
+
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- aggregate over ranks: max time, summed work
+    ms, total_apps = replicas.aggregate(ms_local, apps, world)
+    e2e_s, total_e2e_apps = replicas.aggregate(e2e_s_local, e2e_apps, world)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    value = total_apps * N / (ms * 1e-3) / 1e9
+    e2e_value = total_e2e_apps * N / e2e_s / 1e9
+    peak, peak_src = measured_peaks()
+    bps = BYTES_PER_SITE if prec == "c128" else BYTES_PER_SITE_C64
+    per_kernel = {}
+    for name, (n, kms) in kern.items():
+        if n:
+            per_kernel[name] = {"launches": n, "avg_us": 1e3 * kms / n, "total_ms": kms}
+            if name in bps:
+                per_kernel[name]["alg_GBps"] = bps[name] * N / (1e-3 * kms / n) / 1e9
+    tot_k = sum(v["total_ms"] for v in per_kernel.values())
+    for v in per_kernel.values():
+        v["share"] = v["total_ms"] / tot_k
+    dom = max((k for k in per_kernel if k in bps), key=lambda k: per_kernel[k]["total_ms"])
+    achieved = per_kernel[dom]["alg_GBps"]
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "alg_bytes_per_site": bps[dom],
+                "how": "library CUDA events around every launch of the kernel on its stream during the same step (no graph replay)"}
+    ms_per_step = ms / args.steps
+    # fixed-count PCG iteration cost inside the timed region (graph replay): all four kernels of an iteration
+    cg_share = sum(per_kernel[k]["total_ms"] for k in ("mdagm", "cg_axpy", "precond", "cg_dupdate") if k in per_kernel) / tot_k
+    us_per_iter = 1e3 * ms_per_step * cg_share / (2 * I)
+    cb_dt, cb_apps, cb_threads = oracle_step_sample(L, Ntau, c["seed"], args.ref_cg_iters)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if prec == "c128" else "f32", "data": "synthetic", "config": workload_config(args, L, Ntau, I),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
+            "gpu_launches": launches, "roofline": roofline,
+            "cpu_baseline": {"value": cb_apps * N / cb_dt / 1e9, "unit": UNIT, "cores": cb_threads, "kind": "oracle",
+                             "sample": f"one step on the same lattice with fixed-count CG cut to {args.ref_cg_iters} iterations per solve "
+                                       f"({cb_apps} M^+M), {cb_dt:.1f} s"},
+            "cg_us_per_iter": us_per_iter, "cg_iters_per_s": 1e6 / us_per_iter, "cg_ms_per_solve_fixed": us_per_iter * I * 1e-3,
+            "ms_per_trajectory_step": ms_per_step, "kernels": per_kernel, "mdagm_sweep": sweep,
+            "dH": r["H1"] - r["H0"]}
+    print(json.dumps(line))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def mdagm_sweep(g, torch, dev, L, Ntau, prec, nbuf=8, reps=25):
+    """M^+M alone: cold = rotate nbuf distinct (in, out) pairs so every launch streams from HBM; warm = one pair."""
+    N = L * L * Ntau
+    ins = [g.new_vec() for _ in range(nbuf)]
+    outs = [g.new_vec() for _ in range(nbuf)]
+    for v in ins:
+        v.copy_(torch.randn(v.shape, dtype=v.dtype, device=dev))
+    res = {}
+    for mode in ("cold", "warm"):
+        for i in range(nbuf):
+            g.apply_MdagM(ins[i], outs[i])
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        n = 0
+        for _ in range(reps):
+            for i in range(nbuf):
+                j = i if mode == "cold" else 0
+                g.apply_MdagM(ins[j], outs[j]); n += 1
+        e1.record()
+        torch.cuda.synchronize()
+        us = 1e3 * e0.elapsed_time(e1) / n
+        bps = 48.0 if prec == "c128" else 24.0
+        res[mode] = {"us": us, "Gsite_per_s": N / us / 1e3, "alg_GBps": bps * N / us / 1e3}
+    return res
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number (1-5); 4 = L=48, Ntau=480")
+    ap.add_argument("--cg-iters", type=int, default=500, help="fixed PCG iterations per solve (PAPER.md:348)")
+    ap.add_argument("--ref-cg-iters", type=int, default=2, help="PCG iterations per solve of the CPU-oracle sample")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--prec", default="c128", choices=["c128", "c64"])
+    ap.add_argument("--no-sweep", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

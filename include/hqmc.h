@@ -114,6 +114,9 @@ int hqmc_leapfrog_trajectory(hqmc_ctx *ctx, double *d_theta, double *d_p, const 
 /* HOST-buffer variants (pageable or pinned host memory; the copies run inside the call on the
  * context's stream and the call returns after the result has landed in h_out / h_x). */
 int hqmc_apply_MdagM_host(hqmc_ctx *ctx, const void *h_in, void *h_out);
+/* Pseudofermion refresh from host buffers (PAPER.md:185 step i): copies h_theta (may be NULL: keep the
+ * context's theta) and h_eta to the device, phi = M^+(theta) eta, copies phi to h_phi. */
+int hqmc_refresh_host(hqmc_ctx *ctx, const double *h_theta, const void *h_eta, void *h_phi);
 int hqmc_cg_solve_host(hqmc_ctx *ctx, const double *h_theta, const void *h_rhs, void *h_x, double tol,
                        long long max_iter, long long *iters_out, double *relres_out);
 int hqmc_leapfrog_trajectory_host(hqmc_ctx *ctx, double *h_theta, double *h_p, const void *h_pf, int nsteps,

@@ -99,6 +99,21 @@ extern "C" int hqmc_apply_MdagM_host(hqmc_ctx *c, const void *h_in, void *h_out)
     return HQMC_OK;
 }
 
+extern "C" int hqmc_refresh_host(hqmc_ctx *c, const double *h_theta, const void *h_eta, void *h_phi) {
+    if (!c || !h_eta || !h_phi) return HQMC_EINVAL;
+    const size_t vb = c->N * c->esz;
+    if (h_theta) {
+        CUDA_TRY(cudaMemcpyAsync(c->d_theta, h_theta, sizeof(double) * 2 * c->N, cudaMemcpyHostToDevice, c->stream));
+        HQ_TRY(hqmc_set_theta(c, c->d_theta));
+    }
+    if (!c->theta_set) { g_last_error = "no theta"; return HQMC_EINVAL; }
+    CUDA_TRY(cudaMemcpyAsync(c->d_d, h_eta, vb, cudaMemcpyHostToDevice, c->stream));
+    HQ_TRY(hqmc_apply_Mdag(c, c->d_d, c->d_phi));
+    CUDA_TRY(cudaMemcpyAsync(h_phi, c->d_phi, vb, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return HQMC_OK;
+}
+
 extern "C" int hqmc_cg_solve_host(hqmc_ctx *c, const double *h_theta, const void *h_rhs, void *h_x, double tol,
                                   long long max_iter, long long *iters_out, double *relres_out) {
     if (!c || !h_rhs || !h_x || max_iter < 0) return HQMC_EINVAL;

@@ -23,7 +23,7 @@ KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
-    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_apply_MdagM_host", "hqmc_cg_solve_host",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
@@ -177,6 +177,11 @@ class HQMC:
         assert h_in.dtype == self.np_cdtype and h_out.dtype == self.np_cdtype and h_in.size == self.N == h_out.size
         _check(_lib.hqmc_apply_MdagM_host(self._ctx, h_in.ctypes.data_as(C.c_void_p), h_out.ctypes.data_as(C.c_void_p)))
         return h_out
+
+    def refresh_host(self, h_theta, h_eta, h_phi):
+        th = h_theta.ctypes.data_as(C.c_void_p) if h_theta is not None else None
+        _check(_lib.hqmc_refresh_host(self._ctx, th, h_eta.ctypes.data_as(C.c_void_p), h_phi.ctypes.data_as(C.c_void_p)))
+        return h_phi
 
     def cg_solve_host(self, h_theta, h_rhs, h_x, tol=1e-10, max_iter=1000000):
         it, rel = C.c_longlong(0), C.c_double(0.0)

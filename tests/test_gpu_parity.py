@@ -110,7 +110,7 @@ def test_cg_solution_and_iterations(hq, L, Nt, seed, W):
 @pytest.mark.parametrize("L,Nt,seed", [(4, 8, 0), (6, 10, 1), (12, 14, 2), (50, 4, 5)])
 @pytest.mark.parametrize("compact", [True, False])
 def test_forces_and_energies(hq, L, Nt, seed, compact):
-    o, g, theta = setup(hq, L, Nt, seed, c_tau=1.3, K=0.7, compact=compact)
+    o, g, theta = setup(hq, L, Nt, seed, c_tau=1.3, K=0.7, compact=compact, W=min(6, Nt - 1))
     X = inputs.complex_gaussian((Nt, L, L), seed + 10, inputs.STREAM_VEC)
     phi = inputs.complex_gaussian((Nt, L, L), seed + 11, inputs.STREAM_VEC)
     p = inputs.momenta(L, Nt, seed)
