@@ -132,8 +132,11 @@ enum { HQMC_K_MDAGM = 0, HQMC_K_AXPY = 1, HQMC_K_PRECOND = 2, HQMC_K_DUPDATE = 3
 int hqmc_set_profiling(hqmc_ctx *ctx, int on);
 int hqmc_reset_stats(hqmc_ctx *ctx);
 int hqmc_get_kernel_stats(hqmc_ctx *ctx, int which, long long *launches_out, double *ms_out);
-/* Tuning knob: slices per CTA of the fused M^+M kernel (0 = library default). */
+/* Tuning knobs.  hqmc_set_time_tile: slices per CTA of the fused M^+M kernel (0 = library default: one CTA per SM
+ * with the slices dealt out evenly).  hqmc_set_mdagm_kernel: 0 = streaming kernel (TMA bulk copies, packed link
+ * phases; default where its staging buffers fit shared memory, L <= 48 in complex128), 1 = register-only kernel. */
 int hqmc_set_time_tile(hqmc_ctx *ctx, int slices_per_cta);
+int hqmc_set_mdagm_kernel(hqmc_ctx *ctx, int which);
 
 const char *hqmc_strerror(int status);
 const char *hqmc_last_error(void); /* text of the last CUDA error seen by this thread, or "" */

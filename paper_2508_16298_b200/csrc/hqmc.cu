@@ -64,6 +64,10 @@ template <typename T> static int set_attrs(hqmc_ctx *c) {
         CUDA_TRY(cudaFuncSetAttribute(k_mdagm<T, B, M, true>, attr, smem));
         CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, false>, attr, smem));
         CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, true>, attr, smem));
+        if (c->use_stream) {
+            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_stream<T, false>, attr, (int)c->stream_smem));
+            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_stream<T, true>, attr, (int)c->stream_smem));
+        }
         return HQMC_OK;
     });
 }
@@ -88,10 +92,15 @@ template <typename T> static int auto_time_tile(hqmc_ctx *c) {
 // ---------------------------------------------------------------------------------------------------
 template <typename T> static int do_phase(hqmc_ctx *c, const double *p, double two_eps) {
     typedef typename Cx<T>::type T2;
-    if (p) return launch(c, HQMC_K_PHASE, k_phase<T, true>, dim3(c->grid_ew), dim3(256), 0, c->g, c->d_theta, p, two_eps,
-                         (T2 *)c->d_ph, c->th_full, c->th_half);
-    return launch(c, HQMC_K_PHASE, k_phase<T, false>, dim3(c->grid_ew), dim3(256), 0, c->g, c->d_theta, (const double *)nullptr,
-                  0.0, (T2 *)c->d_ph, c->th_full, c->th_half);
+    typedef typename PhasePack<T>::word W;
+    if (p) HQ_TRY(launch(c, HQMC_K_PHASE, k_phase<T, true>, dim3(c->grid_ew), dim3(256), 0, c->g, c->d_theta, p, two_eps,
+                         (T2 *)c->d_ph, c->th_full, c->th_half));
+    else HQ_TRY(launch(c, HQMC_K_PHASE, k_phase<T, false>, dim3(c->grid_ew), dim3(256), 0, c->g, c->d_theta, (const double *)nullptr,
+                       0.0, (T2 *)c->d_ph, c->th_full, c->th_half));
+    if (c->use_stream)
+        HQ_TRY(launch(c, HQMC_K_PHASE, k_phase_pack<T>, dim3(c->grid_ew), dim3(256), 0, c->g, (const double *)c->d_theta,
+                      (W *)c->d_packed, c->th_full, c->th_half));
+    return HQMC_OK;
 }
 
 template <typename T> static int do_apply_M(hqmc_ctx *c, const void *in, void *out, int dagger) {
@@ -103,8 +112,21 @@ template <typename T> static int do_apply_M(hqmc_ctx *c, const void *in, void *o
     });
 }
 
+template <typename T> static int do_mdagm_stream(hqmc_ctx *c, const void *in, void *out, bool dot, const CgState *st) {
+    typedef typename Cx<T>::type T2;
+    typedef typename PhasePack<T>::word W;
+    int G = c->time_tile > 0 ? (c->g.Nt + c->time_tile - 1) / c->time_tile : (c->g.Nt < c->n_sm ? c->g.Nt : c->n_sm);
+    c->grid_mdagm = G;
+    if (dot)
+        return launch(c, HQMC_K_MDAGM, k_mdagm_stream<T, true>, dim3(G), dim3(c->cfg.threads), c->stream_smem, c->g,
+                      (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, c->d_part_dOd, st);
+    return launch(c, HQMC_K_MDAGM, k_mdagm_stream<T, false>, dim3(G), dim3(c->cfg.threads), c->stream_smem, c->g,
+                  (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st);
+}
+
 template <typename T> static int do_mdagm(hqmc_ctx *c, const void *in, void *out, bool dot, const CgState *st) {
     typedef typename Cx<T>::type T2;
+    if (c->use_stream && c->stream_on) return do_mdagm_stream<T>(c, in, out, dot, st);
     const int Tt = c->time_tile;
     const int grid = (c->g.Nt + Tt - 1) / Tt;
     c->grid_mdagm = grid;

@@ -95,6 +95,24 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     do { cudaError_t e = cudaMalloc((void **)&(ptr), (bytes));                                                    \
          if (e != cudaSuccess) { g_last_error = std::string("cudaMalloc: ") + cudaGetErrorString(e); return fail(HQMC_ENOMEM); } } while (0)
     ALLOC(c->d_theta, tb); ALLOC(c->d_ph, 2 * c->N * c->esz);
+    {   // streaming M^+M kernel: one thread per 2x2 block and its staging buffers must fit one SM's shared memory
+        const size_t need = (prm->prec == HQMC_C128) ? StreamSmem<double>(c->g.Vs, c->cfg.threads).total : StreamSmem<float>(c->g.Vs, c->cfg.threads).total;
+        c->stream_smem = need;
+        c->use_stream = (c->cfg.bpt == 1) && need <= (size_t)prop.sharedMemPerBlockOptin && (size_t)c->g.Vs * 16 < (1u << 20);
+        c->stream_on = c->use_stream;
+    }
+    if (c->use_stream) {
+        ALLOC(c->d_packed, 2 * c->N * 8);
+        ALLOC(c->d_tab, sizeof(double2) * 2 * HQMC_PHASE_K);
+        std::vector<double2> tab((size_t)2 * HQMC_PHASE_K);
+        for (int s2 = 0; s2 < 2; ++s2)
+            for (int k = 0; k < HQMC_PHASE_K; ++k) {
+                const double ang = 2.0 * M_PI * (double)k / (double)HQMC_PHASE_K, sc = s2 ? c->th_full : c->th_half;
+                tab[(size_t)s2 * HQMC_PHASE_K + k] = make_double2(sc * std::cos(ang), sc * std::sin(ang));
+            }
+        cudaError_t e = cudaMemcpy(c->d_tab, tab.data(), sizeof(double2) * tab.size(), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { g_last_error = cudaGetErrorString(e); return fail(HQMC_ECUDA); }
+    }
     ALLOC(c->d_r, vb); ALLOC(c->d_z, vb); ALLOC(c->d_d, vb); ALLOC(c->d_Od, vb); ALLOC(c->d_X, vb); ALLOC(c->d_phi, vb);
     ALLOC(c->d_p, tb); ALLOC(c->d_force, tb);
     ALLOC(c->d_part_dOd, sizeof(double) * HQMC_MAX_PART); ALLOC(c->d_part_rr, sizeof(double) * HQMC_MAX_PART);
@@ -109,6 +127,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     if (st != HQMC_OK) return fail(st);
     st = DISPATCH_T(c, auto_time_tile<double>(c), auto_time_tile<float>(c));
     if (st != HQMC_OK) return fail(st);
+    if (c->use_stream) c->time_tile = 0;
     st = build_default_taps(c);
     if (st != HQMC_OK) return fail(st);
     *out = c;
@@ -121,7 +140,7 @@ extern "C" int hqmc_destroy(hqmc_ctx *c) {
     if (c->cg_graph) cudaGraphExecDestroy(c->cg_graph);
     for (auto &ep : c->pending) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (auto &ep : c->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-    void *ptrs[] = {c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
+    void *ptrs[] = {c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
                     c->d_part_rr, c->d_part_rz[0], c->d_part_rz[1], c->d_part_misc, c->d_state, c->d_scal};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (c->h_state) cudaFreeHost(c->h_state);
@@ -201,10 +220,20 @@ extern "C" int hqmc_get_kernel_stats(hqmc_ctx *c, int which, long long *launches
 }
 extern "C" int hqmc_set_time_tile(hqmc_ctx *c, int tt) {
     if (!c || tt < 0 || tt > c->g.Nt) return HQMC_EINVAL;
-    if (tt == 0) return DISPATCH_T(c, auto_time_tile<double>(c), auto_time_tile<float>(c));
+    if (tt == 0) {
+        if (c->use_stream && c->stream_on) { c->time_tile = 0; return HQMC_OK; }   // one CTA per SM, slices dealt out evenly
+        return DISPATCH_T(c, auto_time_tile<double>(c), auto_time_tile<float>(c));
+    }
     if ((c->g.Nt + tt - 1) / tt > HQMC_MAX_PART) return HQMC_EINVAL;
     c->time_tile = tt;
     return HQMC_OK;
+}
+extern "C" int hqmc_set_mdagm_kernel(hqmc_ctx *c, int which) {
+    if (!c || which < 0 || which > 1) return HQMC_EINVAL;
+    if (which == 0 && !c->use_stream) return HQMC_EINVAL;
+    c->stream_on = (which == 0);
+    if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+    return hqmc_set_time_tile(c, 0);
 }
 
 extern "C" const char *hqmc_strerror(int s) {

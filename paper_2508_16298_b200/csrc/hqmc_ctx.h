@@ -13,6 +13,7 @@
 #include "cg_kernels.cuh"
 #include "force_kernels.cuh"
 #include "kernels.cuh"
+#include "mdagm_stream.cuh"
 
 namespace hqmc {
 
@@ -54,6 +55,11 @@ struct hqmc_ctx {
     // device memory owned by the context
     double *d_theta;     // copy of the gauge field
     void *d_ph;          // phase table [Nt][2][L][L] complex
+    void *d_packed;      // packed link phases [Nt][4][nb][2] (8 B each) for the streaming M^+M kernel
+    double2 *d_tab;      // [2][1024] tanh(a) e^{i k delta} (half step, full step)
+    bool stream_on;      // runtime switch (hqmc_set_mdagm_kernel)
+    bool use_stream;     // streaming kernel usable (BPT == 1 and its shared memory fits)
+    size_t stream_smem;
     void *d_r, *d_z, *d_d, *d_Od, *d_X, *d_phi;   // CG vectors, trajectory solution / pseudofermion
     double *d_p, *d_force;                        // host-variant staging
     double *d_part_dOd, *d_part_rr, *d_part_rz[2], *d_part_misc;

@@ -1,0 +1,362 @@
+// mdagm_stream.cuh -- streaming fused O v = M^+ M v kernel (sm_100a): TMA bulk copies + packed link phases.
+//
+//   w_t = v_t - sigma_{t-1} B_{t-1} v_{t-1};   out_t = w_t - sigma_t B_t w_{t+1}      (Eq.8, 284-314)
+//
+// One CTA owns a run of consecutive time slices [t0, t1) of the WHOLE spatial lattice (one thread per 2x2
+// block of sites, block_engine.cuh).  What is new relative to k_mdagm (kernels.cuh):
+//  * every global access is a 1-D TMA bulk copy (cp.async.bulk, SASS UBLKCP) issued one slice ahead by one
+//    thread and completed on an mbarrier: v_{t+1} and the link phases of slice t+1 land in shared memory while
+//    slice t is being swept, and out_t leaves through a staged bulk store -- no thread ever waits on HBM;
+//  * link phases are streamed in a PACKED 8-byte form (PhasePack below) instead of 16-byte complex numbers, so
+//    one M^+M moves 16 (v) + 16 (two links) + 16 (out) = 48 B/site, the algorithmic minimum of DESIGN.md;
+//  * the grid is one CTA per SM with the slices dealt out as evenly as possible (480 slices over 148 SMs =
+//    36 runs of 4 + 112 runs of 3) instead of ceil(Nt/Tt) equal tiles.
+#pragma once
+#include <cstdint>
+
+#include "kernels.cuh"
+
+namespace hqmc {
+
+// ------------------------------------------------------------------------------------------------
+// PhasePack: 8 bytes per link.
+// double:  theta = k*delta + r, delta = 2 pi / 1024, |r| <= delta/2.  The word holds sin(r) as an fp64 with its
+//          10 low mantissa bits replaced by k (sin r < 2^-8, so the absolute error of the stored sine is
+//          <= 2^-8 * 2^-43 = 4.4e-16 ... 1.1e-16 after rounding to nearest -- one ulp of a unit phase).
+//          Decode: cos r = 1 - q/2 - q^2/8 (q = sin^2 r <= 9.5e-6, next term 5e-17), then one complex
+//          multiply with the table entry  tanh(a) e^{i k delta}  (shared memory, 1024 entries per scale a).
+// float:   the scaled phase itself as float2 (8 bytes), no decoding.
+// ------------------------------------------------------------------------------------------------
+#define HQMC_PHASE_K 1024
+
+template <typename T> struct PhasePack;
+template <> struct PhasePack<double> {
+    typedef unsigned long long word;
+    static __device__ __forceinline__ word pack(double theta, double /*scale*/) {
+        const double inv_delta = 162.97466172610083;       // 1024 / (2 pi)
+        const double d_hi = 0.006135923151542565;           // fp64(2 pi / 1024)
+        const double d_lo = 2.391888279584674e-19;           // 2 pi / 1024 - d_hi
+        double kf = rint(theta * inv_delta);
+        double r = fma(-kf, d_hi, theta);
+        r = fma(-kf, d_lo, r);
+        long long k = (long long)kf;
+        double s = sin(r);
+        unsigned long long u = (unsigned long long)__double_as_longlong(s);
+        u = (u + 512ull) & ~1023ull;                         // round the mantissa to 43 bits
+        return u | (unsigned long long)(k & 1023ll);
+    }
+    static __device__ __forceinline__ double2 decode(word u, const double2 *__restrict__ tab) {
+        const unsigned k = (unsigned)u & 1023u;
+        const double sr = __longlong_as_double((long long)(u & ~1023ull));
+        const double q = sr * sr;
+        const double cr = fma(q, fma(q, -0.125, -0.5), 1.0);
+        const double2 t = tab[k];
+        double2 P;
+        P.x = fma(-t.y, sr, t.x * cr);
+        P.y = fma(t.x, sr, t.y * cr);
+        return P;
+    }
+};
+template <> struct PhasePack<float> {
+    typedef float2 word;
+    static __device__ __forceinline__ word pack(double theta, double scale) {
+        double s, c;
+        sincos(theta, &s, &c);
+        return make_float2((float)(scale * c), (float)(scale * s));
+    }
+    static __device__ __forceinline__ float2 decode(word u, const double2 *) { return u; }
+};
+
+// Position of bond (mu, y, x) of a slice in the block-major packed layout [4 pairs][nb blocks][2]:
+// pair 0 = family 4 (y-bonds, y odd), 1 = family 3 (y-bonds, y even), 2 = family 2 (x-bonds, x odd),
+// 3 = family 1 (x-bonds, x even) -- the order in which block_engine.cuh's BlockIdx lists p4, p3, p2, p1.
+__device__ __forceinline__ int packed_slot(const Geo &g, int mu, int y, int x) {
+    int j, bx, by, e;
+    if (mu == 1) {
+        if (x & 1) { bx = (x - 1) >> 1; e = 0; } else { bx = (x >> 1) - 1; if (bx < 0) bx = g.h - 1; e = 1; }
+        if (y & 1) { j = 0; by = (y - 1) >> 1; } else { j = 1; by = y >> 1; }
+    } else {
+        by = y >> 1; e = y & 1;
+        if (x & 1) { j = 2; bx = (x - 1) >> 1; } else { j = 3; bx = x >> 1; }
+    }
+    return ((j * g.nb) + by * g.h + bx) * 2 + e;
+}
+
+// S1 (streaming form): packed[t][4][nb][2] from theta[t][2][L][L]; a = dtau*t for family 1, dtau*t/2 otherwise.
+template <typename T>
+__global__ void k_phase_pack(Geo g, const double *__restrict__ theta, typename PhasePack<T>::word *__restrict__ packed,
+                             double th_full, double th_half) {
+    const size_t per = (size_t)2 * g.Vs, n = per * g.Nt;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t t = i / per;
+        const int r = (int)(i - t * per);
+        const int mu = r / g.Vs, s = r - mu * g.Vs, y = s / g.L, x = s - y * g.L;
+        const double sc = (mu == 0 && (x & 1) == 0) ? th_full : th_half;
+        packed[t * per + packed_slot(g, mu, y, x)] = PhasePack<T>::pack(theta[i], sc);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// mbarrier / TMA bulk-copy helpers (PTX; SASS: SYNCS.*, UBLKCP)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *dst_gmem, const void *src_smem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// ------------------------------------------------------------------------------------------------
+// Lean single-block-per-thread engine for the streaming kernel: everything a thread needs is a handful of
+// shared-memory element offsets computed once; the four re-alignments of block_engine.cuh are written out
+// with compile-time buffer parity so that no register is ever moved (the compiler renames).
+// Threads beyond nb (ragged last warp) run the same code on a private dummy exchange slot and never store.
+// ------------------------------------------------------------------------------------------------
+struct LeanIdx {
+    int o0, o1, o2, o3;          // OO-layout site offsets inside a slice: (xa,ya) (xb,ya) (xa,yb) (xb,yb)
+    int d_yd, d_xd, d_xu, d_yu;  // exchange destinations
+    int q;
+    bool act;
+};
+__device__ __forceinline__ void make_lean(const Geo &g, int q, LeanIdx &b) {
+    b.q = q; b.act = q < g.nb;
+    const int qq = b.act ? q : 0;
+    const int by = qq / g.h, bx = qq - by * g.h, L = g.L;
+    const int xa = 2 * bx + 1, xb = (xa + 1 == L) ? 0 : xa + 1;
+    const int ya = 2 * by + 1, yb = (ya + 1 == L) ? 0 : ya + 1;
+    b.o0 = ya * L + xa; b.o1 = ya * L + xb; b.o2 = yb * L + xa; b.o3 = yb * L + xb;
+    const int byp = (by + 1 == g.h) ? 0 : by + 1, bym = (by == 0) ? g.h - 1 : by - 1;
+    const int bxp = (bx + 1 == g.h) ? 0 : bx + 1, bxm = (bx == 0) ? g.h - 1 : bx - 1;
+    b.d_yd = b.act ? bx + g.h * byp : q; b.d_xd = b.act ? bxp + g.h * by : q;
+    b.d_xu = b.act ? bxm + g.h * by : q; b.d_yu = b.act ? bx + g.h * bym : q;
+}
+
+// ex: [2 parities][2 slots][nbp] elements.  KIND 0: OO->OE (y down), 1: OE->EE (x down), 2: EE->OE (x up), 3: OE->OO (y up).
+// v0..v3 are passed and returned in the layout order (xa,ya) (xb,ya) (xa,yb) (xb,yb) of the CURRENT alignment.
+template <int KIND, int PAR, typename T2, typename Hook>
+__device__ __forceinline__ void lean_realign(T2 *__restrict__ ex, int nbp, const LeanIdx &b, T2 &v0, T2 &v1, T2 &v2, T2 &v3, Hook &&hook) {
+    T2 *s0 = ex + (size_t)(PAR * 2) * nbp, *s1 = s0 + nbp;
+    if (KIND == 0)      { s0[b.d_yd] = v2; s1[b.d_yd] = v3; }
+    else if (KIND == 1) { s0[b.d_xd] = v1; s1[b.d_xd] = v3; }
+    else if (KIND == 2) { s0[b.d_xu] = v0; s1[b.d_xu] = v2; }
+    else                { s0[b.d_yu] = v0; s1[b.d_yu] = v1; }
+    __syncthreads();
+    hook();
+    const T2 r0 = s0[b.q], r1 = s1[b.q];
+    if (KIND == 0)      { v2 = v0; v3 = v1; v0 = r0; v1 = r1; }
+    else if (KIND == 1) { v1 = v0; v3 = v2; v0 = r0; v2 = r1; }
+    else if (KIND == 2) { v0 = v1; v2 = v3; v1 = r0; v3 = r1; }
+    else                { v0 = v2; v1 = v3; v2 = r0; v3 = r1; }
+}
+
+template <typename T2> struct LeanPh { T2 a4, b4, a3, b3, a2, b2, a1, b1; };   // p4[0], p4[1], p3[0], ...
+
+// v <- prod_k (1 + t_k T_k) v  (B without its scalar C), OO layout in and out; hook runs on every thread right
+// after the first barrier.
+template <typename T2, typename Hook>
+__device__ __forceinline__ void lean_apply_B(T2 *__restrict__ ex, int nbp, const LeanIdx &b, const LeanPh<T2> &P,
+                                             T2 &v0, T2 &v1, T2 &v2, T2 &v3, Hook &&hook) {
+    rot(v0, v2, P.a4); rot(v1, v3, P.b4);
+    lean_realign<0, 0>(ex, nbp, b, v0, v1, v2, v3, hook);
+    rot(v0, v2, P.a3); rot(v1, v3, P.b3);
+    rot(v0, v1, P.a2); rot(v2, v3, P.b2);
+    lean_realign<1, 1>(ex, nbp, b, v0, v1, v2, v3, []() {});
+    rot(v0, v1, P.a1); rot(v2, v3, P.b1);
+    lean_realign<2, 0>(ex, nbp, b, v0, v1, v2, v3, []() {});
+    rot(v0, v1, P.a2); rot(v2, v3, P.b2);
+    rot(v0, v2, P.a3); rot(v1, v3, P.b3);
+    lean_realign<3, 1>(ex, nbp, b, v0, v1, v2, v3, []() {});
+    rot(v0, v2, P.a4); rot(v1, v3, P.b4);
+}
+
+template <typename T> struct PackLoad;
+template <> struct PackLoad<double> {
+    static __device__ __forceinline__ void pair(const unsigned char *p, const double2 *tab, double2 &A, double2 &B) {
+        const ulonglong2 w = *reinterpret_cast<const ulonglong2 *>(p);
+        A = PhasePack<double>::decode(w.x, tab); B = PhasePack<double>::decode(w.y, tab);
+    }
+};
+template <> struct PackLoad<float> {
+    static __device__ __forceinline__ void pair(const unsigned char *p, const double2 *, float2 &A, float2 &B) {
+        const float4 w = *reinterpret_cast<const float4 *>(p);
+        A = make_float2(w.x, w.y); B = make_float2(w.z, w.w);
+    }
+};
+template <typename T>
+__device__ __forceinline__ void lean_load_phases(const unsigned char *pbuf, const double2 *tab, int nb, int q, LeanPh<typename Cx<T>::type> &P) {
+    const unsigned char *p = pbuf + (size_t)q * 16;
+    const size_t st = (size_t)nb * 16;
+    PackLoad<T>::pair(p, tab, P.a4, P.b4);
+    PackLoad<T>::pair(p + st, tab, P.a3, P.b3);
+    PackLoad<T>::pair(p + 2 * st, tab, P.a2, P.b2);
+    PackLoad<T>::pair(p + 3 * st, tab + HQMC_PHASE_K, P.a1, P.b1);
+}
+
+template <typename T> struct StreamSmem {
+    // byte offsets inside dynamic shared memory (nbp = threads per CTA >= nb)
+    size_t tab, vbuf, pbuf, obuf, exch, red, bars, total;
+    __host__ __device__ StreamSmem(int Vs, int nbp) {
+        typedef typename Cx<T>::type T2;
+        size_t o = 0;
+        tab = o;  o += (sizeof(T) == 8) ? (size_t)2 * HQMC_PHASE_K * sizeof(double2) : 0;
+        vbuf = o; o += (size_t)Vs * sizeof(T2);
+        pbuf = o; o += (size_t)2 * Vs * 8;
+        obuf = o; o += (size_t)Vs * sizeof(T2);
+        exch = o; o += (size_t)4 * nbp * sizeof(T2);
+        red = o;  o += 32 * sizeof(double);
+        bars = o; o += 4 * sizeof(uint64_t);
+        total = o;
+    }
+};
+
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    mbar_expect_tx(bar, bytes);
+    bulk_g2s(dst, src, bytes, bar);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S5, streaming form.  grid = G CTAs; CTA i owns slices [i*Nt/G, (i+1)*Nt/G); blockDim.x = nb rounded up to 32.
+// packed: [Nt][4][nb][2] PhasePack words;  tab_g: [2][1024] double2 (half step, full step) in global memory.
+// DOT: part[blockIdx] = sum_t ||w_t||^2 over the CTA's slices ( <v, O v> = ||M v||^2 ).
+// Slice bytes must stay below the mbarrier tx-count limit (2^20): checked by the host (use_stream).
+// ------------------------------------------------------------------------------------------------
+template <typename T, bool DOT>
+__global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename PhasePack<T>::word *__restrict__ packed,
+                        const double2 *__restrict__ tab_g, const typename Cx<T>::type *__restrict__ in,
+                        typename Cx<T>::type *__restrict__ out, T C, double *__restrict__ part, const CgState *__restrict__ st) {
+    typedef typename Cx<T>::type T2;
+    if (st != nullptr && *(volatile const int *)&st->done) return;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int nbp = blockDim.x;
+    const StreamSmem<T> lay(g.Vs, nbp);
+    const double2 *tab = reinterpret_cast<const double2 *>(smem_raw + lay.tab);
+    unsigned char *pbuf = smem_raw + lay.pbuf;
+    const T2 *vsm = reinterpret_cast<const T2 *>(smem_raw + lay.vbuf);
+    T2 *osm = reinterpret_cast<T2 *>(smem_raw + lay.obuf);
+    T2 *ex = reinterpret_cast<T2 *>(smem_raw + lay.exch);
+    double *red = reinterpret_cast<double *>(smem_raw + lay.red);
+    uint64_t *bar_v = reinterpret_cast<uint64_t *>(smem_raw + lay.bars), *bar_p = bar_v + 1, *bar_t = bar_v + 2;
+    LeanIdx b;
+    make_lean(g, threadIdx.x, b);
+
+    const int G = gridDim.x;
+    const int t0 = (int)(((long long)blockIdx.x * g.Nt) / G), t1 = (int)(((long long)(blockIdx.x + 1) * g.Nt) / G);
+    if (t0 >= t1) { if (DOT && threadIdx.x == 0) part[blockIdx.x] = 0.0; return; }
+    const uint32_t vbytes = (uint32_t)g.Vs * sizeof(T2), pbytes = (uint32_t)g.Vs * 16;
+    const unsigned char *in_b = reinterpret_cast<const unsigned char *>(in);
+    const unsigned char *pk_b = reinterpret_cast<const unsigned char *>(packed);
+    unsigned char *out_b = reinterpret_cast<unsigned char *>(out);
+    const bool leader = threadIdx.x == 0;
+    uint32_t par_v = 0, par_p = 0;
+    const int tp = (t0 == 0) ? g.Nt - 1 : t0 - 1;
+
+    if (leader) {
+        mbar_init(bar_v, 1); mbar_init(bar_p, 1); mbar_init(bar_t, 1);
+        mbar_fence_init();
+        if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_K * sizeof(double2), bar_t);
+        bulk_load(smem_raw + lay.vbuf, in_b + (size_t)tp * vbytes, vbytes, bar_v);
+        bulk_load(pbuf, pk_b + (size_t)tp * pbytes, pbytes, bar_p);
+    }
+    __syncthreads();                      // barrier inits visible to every thread
+    if (sizeof(T) == 8) mbar_wait(bar_t, 0);
+
+    T2 w0, w1, w2, w3;                    // w_t
+    LeanPh<T2> P;
+    double acc = 0.0;
+
+    // ---- prologue: w_{t0} = v_{t0} - sigma_{tp} C B_{tp} v_{tp}
+    mbar_wait(bar_v, par_v); par_v ^= 1;
+    mbar_wait(bar_p, par_p); par_p ^= 1;
+    w0 = vsm[b.o0]; w1 = vsm[b.o1]; w2 = vsm[b.o2]; w3 = vsm[b.o3];
+    lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
+    lean_apply_B(ex, nbp, b, P, w0, w1, w2, w3, [&]() {
+        if (leader) {
+            bulk_load(smem_raw + lay.vbuf, in_b + (size_t)t0 * vbytes, vbytes, bar_v);
+            bulk_load(pbuf, pk_b + (size_t)t0 * pbytes, pbytes, bar_p);
+        }
+    });
+    {
+        const T sC = (tp == g.Nt - 1) ? C : -C;
+        mbar_wait(bar_v, par_v); par_v ^= 1;
+        mbar_wait(bar_p, par_p); par_p ^= 1;
+        T2 v0 = vsm[b.o0], v1 = vsm[b.o1], v2 = vsm[b.o2], v3 = vsm[b.o3];
+        w0.x = fma(sC, w0.x, v0.x); w0.y = fma(sC, w0.y, v0.y); w1.x = fma(sC, w1.x, v1.x); w1.y = fma(sC, w1.y, v1.y);
+        w2.x = fma(sC, w2.x, v2.x); w2.y = fma(sC, w2.y, v2.y); w3.x = fma(sC, w3.x, v3.x); w3.y = fma(sC, w3.y, v3.y);
+        lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
+    }
+
+    for (int t = t0; t < t1; ++t) {
+        const int tn = (t + 1 == g.Nt) ? 0 : t + 1;
+        const T sC = (t == g.Nt - 1) ? C : -C;
+        const bool more = (t + 1 < t1);
+        // v = B_t v_t / C; v_t is still in vbuf (it is refilled only after the first barrier below, by which time
+        // everyone has read it and pbuf) and obuf holds out_{t-1} completely: thread 0 stores it and fetches v_{t+1}
+        // and the phases of slice t+1.
+        T2 v0 = vsm[b.o0], v1 = vsm[b.o1], v2 = vsm[b.o2], v3 = vsm[b.o3];
+        lean_apply_B(ex, nbp, b, P, v0, v1, v2, v3, [&]() {
+            if (leader) {
+                if (t > t0) { bulk_s2g(out_b + (size_t)(t - 1) * vbytes, osm, vbytes); bulk_commit(); }
+                bulk_load(smem_raw + lay.vbuf, in_b + (size_t)tn * vbytes, vbytes, bar_v);
+                if (more) bulk_load(pbuf, pk_b + (size_t)tn * pbytes, pbytes, bar_p);
+            }
+        });
+        mbar_wait(bar_v, par_v); par_v ^= 1;
+        T2 n0 = vsm[b.o0], n1 = vsm[b.o1], n2 = vsm[b.o2], n3 = vsm[b.o3];       // v_{t+1}
+        T2 q0, q1, q2, q3;                                                         // w_{t+1}, then B_t w_{t+1}
+        q0.x = fma(sC, v0.x, n0.x); q0.y = fma(sC, v0.y, n0.y); q1.x = fma(sC, v1.x, n1.x); q1.y = fma(sC, v1.y, n1.y);
+        q2.x = fma(sC, v2.x, n2.x); q2.y = fma(sC, v2.y, n2.y); q3.x = fma(sC, v3.x, n3.x); q3.y = fma(sC, v3.y, n3.y);
+        const T2 k0 = q0, k1 = q1, k2 = q2, k3 = q3;                               // keep w_{t+1}
+        // The store of out_{t-1} must have finished READING obuf before obuf is rewritten below: thread 0 waits
+        // for that before the first barrier of this sweep sequence.
+        if (leader) bulk_wait_read0();
+        lean_apply_B(ex, nbp, b, P, q0, q1, q2, q3, []() {});
+        if (DOT && b.act)
+            acc += ((double)w0.x * w0.x + (double)w0.y * w0.y) + ((double)w1.x * w1.x + (double)w1.y * w1.y) +
+                   ((double)w2.x * w2.x + (double)w2.y * w2.y) + ((double)w3.x * w3.x + (double)w3.y * w3.y);
+        q0.x = fma(sC, q0.x, w0.x); q0.y = fma(sC, q0.y, w0.y); q1.x = fma(sC, q1.x, w1.x); q1.y = fma(sC, q1.y, w1.y);
+        q2.x = fma(sC, q2.x, w2.x); q2.y = fma(sC, q2.y, w2.y); q3.x = fma(sC, q3.x, w3.x); q3.y = fma(sC, q3.y, w3.y);
+        w0 = k0; w1 = k1; w2 = k2; w3 = k3;
+        if (b.act) { osm[b.o0] = q0; osm[b.o1] = q1; osm[b.o2] = q2; osm[b.o3] = q3; }
+        fence_async_smem();               // my obuf writes -> visible to the async proxy (the store is issued after the next barrier)
+        if (more) {
+            mbar_wait(bar_p, par_p); par_p ^= 1;
+            lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
+        }
+    }
+    __syncthreads();
+    if (leader) {
+        bulk_s2g(out_b + (size_t)(t1 - 1) * vbytes, osm, vbytes);
+        bulk_commit();
+        bulk_wait0();
+    }
+    if (DOT) {
+        double s = block_sum(acc, red);
+        if (threadIdx.x == 0) part[blockIdx.x] = s;
+    }
+}
+
+}  // namespace hqmc

@@ -47,9 +47,15 @@ def test_M_Mdag_MdagM(hq, L, Nt, seed):
     assert rel(g.apply_Mdag(dv).cpu().numpy(), o.apply_Mdag(theta, v)) <= 1e-12
     ref = o.apply_MdagM(theta, v)
     assert rel(g.apply_MdagM(dv).cpu().numpy(), ref) <= 1e-12
-    for tt in (1, 2, 3, Nt):          # every time-tile shape incl. ragged last tile and one-CTA-for-all
-        g.set_time_tile(tt)
-        assert rel(g.apply_MdagM(dv).cpu().numpy(), ref) <= 1e-12
+    for which in (0, 1):              # 0: streaming (TMA) kernel where it fits shared memory, 1: register-only kernel
+        try:
+            g.set_mdagm_kernel(which)
+        except hq.HqmcError:
+            assert which == 0 and L > 48
+            continue
+        for tt in (0, 1, 2, 3, Nt):   # default split and every time-tile shape incl. ragged last tile and one-CTA-for-all
+            g.set_time_tile(tt)
+            assert rel(g.apply_MdagM(dv).cpu().numpy(), ref) <= 1e-12, (which, tt)
     g.close()
 
 
