@@ -104,6 +104,82 @@ __global__ void k_precond(Geo g, Taps taps, const typename Cx<T>::type *__restri
     }
 }
 
+// Sliding-window form of the same operator for the common half bandwidth W (compile time): thread = one spatial
+// site, marching through a run of TR consecutive slices with the 2W+1 slices it needs held in registers (a 16-slot
+// ring, three slots of which are loads in flight), so every r element is read once per run (+2W halo per run)
+// instead of 2W+1 times; lanes = consecutive sites, so each load/store instruction moves 32 contiguous elements.
+// Same modes / bookkeeping as k_precond.  grid = (ceil(Vs/128), ceil(Nt/TR)); partial index = y*gridDim.x + x.
+template <typename T, int W>
+__global__ void __launch_bounds__(128) k_precond_win(Geo g, Taps taps, const typename Cx<T>::type *__restrict__ r,
+                                                     typename Cx<T>::type *__restrict__ z, double *__restrict__ part_rz,
+                                                     const double *__restrict__ part_rr, int n_rr, CgState *st, int mode, int TR) {
+    typedef typename Cx<T>::type T2;
+    static_assert(W >= 1 && W <= 6, "ring of 16 slots holds 2W+1 <= 13 live slices + 3 in flight");
+    constexpr int RING = 16, PF = RING - (2 * W + 1);
+    if (mode != 0 && *(volatile const int *)&st->done) return;
+    __shared__ double red[32];
+    const int Vs = g.Vs, Nt = g.Nt;
+    const int s = blockIdx.x * 128 + threadIdx.x;
+    const bool act = s < Vs;
+    const int ta = blockIdx.y * TR, tb = min(ta + TR, Nt);
+    const T2 *rs = r + (act ? s : 0);
+    T2 *zs = z + (act ? s : 0);
+    // r at time index u in [ta - W, tb - 1 + W] (a subset of (-Nt, 2 Nt) because W < Nt), with the antiperiodic
+    // sign; indices past the last slice this run needs are not touched.
+    const int u_max = tb - 1 + W;
+    auto ld = [&](int u) -> T2 {
+        T sg = (T)1;
+        if (u > u_max) { T2 zero; zero.x = (T)0; zero.y = (T)0; return zero; }
+        if (u < 0) { u += Nt; sg = (T)-1; } else if (u >= Nt) { u -= Nt; sg = (T)-1; }
+        T2 v = rs[(size_t)u * Vs];
+        v.x *= sg; v.y *= sg;
+        return v;
+    };
+    T2 ring[RING];
+    // slot of time u: (u - ta + W) mod RING.  Preload times ta-W .. ta+W-1+PF.
+#pragma unroll
+    for (int j = 0; j < 2 * W + PF; ++j) ring[j] = ld(ta - W + j);
+    double acc = 0.0;
+    for (int t = ta; t < tb; t += RING) {
+#pragma unroll
+        for (int j = 0; j < RING; ++j) {
+            const int tt = t + j;
+            if (tt < tb) {
+                ring[(j + 2 * W + PF) % RING] = ld(tt + W + PF);          // in flight for PF steps
+                const T2 c = ring[(j + W) % RING];
+                double zx = taps.p[0] * (double)c.x, zy = taps.p[0] * (double)c.y;
+#pragma unroll
+                for (int m = 1; m <= W; ++m) {
+                    const T2 a = ring[(j + W + m) % RING], b = ring[(j + W - m) % RING];
+                    zx = fma(taps.p[m], (double)a.x + (double)b.x, zx);
+                    zy = fma(taps.p[m], (double)a.y + (double)b.y, zy);
+                }
+                T2 zi; zi.x = (T)zx; zi.y = (T)zy;
+                if (act) {
+                    zs[(size_t)tt * Vs] = zi;
+                    acc += (double)c.x * (double)zi.x + (double)c.y * (double)zi.y;
+                }
+            }
+        }
+    }
+    double sblk = block_sum(acc, red);
+    const int bid = blockIdx.y * gridDim.x + blockIdx.x;
+    if (threadIdx.x == 0 && part_rz != nullptr) part_rz[bid] = sblk;
+    if (mode != 0 && bid == 0) {
+        double rr = sum_partials_warp0(part_rr, n_rr);
+        if (threadIdx.x == 0) {
+            if (mode == 1) {
+                st->bb = rr; st->rr = rr; st->iters = 0;
+                st->done = (rr == 0.0 || st->max_iter <= 0) ? 1 : 0;
+            } else {
+                long long it = st->iters + 1;
+                st->iters = it; st->rr = rr;
+                if ((st->tol2 > 0.0 && rr <= st->tol2 * st->bb) || it >= st->max_iter) st->done = 1;
+            }
+        }
+    }
+}
+
 // beta = <r,z>_new / <r,z>_old;  d = z + beta d   (first: d = z)
 template <typename T>
 __global__ void k_cg_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, const typename Cx<T>::type *__restrict__ z,

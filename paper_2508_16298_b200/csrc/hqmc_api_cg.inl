@@ -11,11 +11,11 @@ template <typename T> static int cg_iteration(hqmc_ctx *c, void *x, int par) {
     typedef typename Cx<T>::type T2;
     HQ_TRY(do_mdagm<T>(c, c->d_d, c->d_Od, true, c->d_state));
     HQ_TRY(launch(c, HQMC_K_AXPY, k_cg_axpy<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_r, (const T2 *)c->d_d,
-                  (const T2 *)c->d_Od, (const double *)c->d_part_rz[par], c->grid_ew, (const double *)c->d_part_dOd,
+                  (const T2 *)c->d_Od, (const double *)c->d_part_rz[par], c->n_part_rz, (const double *)c->d_part_dOd,
                   c->grid_mdagm, c->d_part_rr, (const CgState *)c->d_state));
     HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[par ^ 1], 2));
     HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)c->d_z,
-                  (const double *)c->d_part_rz[par ^ 1], (const double *)c->d_part_rz[par], c->grid_ew, 0,
+                  (const double *)c->d_part_rz[par ^ 1], (const double *)c->d_part_rz[par], c->n_part_rz, 0,
                   (const CgState *)c->d_state));
     return HQMC_OK;
 }
@@ -53,7 +53,7 @@ template <typename T> static int cg_solve_t(hqmc_ctx *c, const void *rhs, void *
                   c->d_part_rr));
     HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[0], 1));
     HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)c->d_z,
-                  (const double *)c->d_part_rz[0], (const double *)c->d_part_rz[0], c->grid_ew, 1, (const CgState *)c->d_state));
+                  (const double *)c->d_part_rz[0], (const double *)c->d_part_rz[0], c->n_part_rz, 1, (const CgState *)c->d_state));
     const bool use_graph = !c->profiling;
     if (use_graph) HQ_TRY(cg_build_graph<T>(c, x));
     long long launched = 0;

@@ -130,6 +130,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     if (c->use_stream) c->time_tile = 0;
     st = build_default_taps(c);
     if (st != HQMC_OK) return fail(st);
+    precond_cfg(c, 0);
     *out = c;
     return HQMC_OK;
 }
@@ -157,6 +158,7 @@ extern "C" int hqmc_set_precond(hqmc_ctx *c, int W, const double *taps_host) {
     if (W == 0) c->taps.p[0] = taps_host ? taps_host[0] : 1.0;
     else for (int i = 0; i <= W; ++i) c->taps.p[i] = taps_host[i];
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }   // taps are baked into the graph
+    precond_cfg(c, 0);
     return HQMC_OK;
 }
 
@@ -226,6 +228,12 @@ extern "C" int hqmc_set_time_tile(hqmc_ctx *c, int tt) {
     }
     if ((c->g.Nt + tt - 1) / tt > HQMC_MAX_PART) return HQMC_EINVAL;
     c->time_tile = tt;
+    return HQMC_OK;
+}
+extern "C" int hqmc_set_precond_tile(hqmc_ctx *c, int slices_per_run) {
+    if (!c || slices_per_run < 0) return HQMC_EINVAL;
+    if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+    precond_cfg(c, slices_per_run);
     return HQMC_OK;
 }
 extern "C" int hqmc_set_mdagm_kernel(hqmc_ctx *c, int which) {

@@ -70,6 +70,8 @@ struct hqmc_ctx {
     bool theta_set;
     // grids
     int grid_ew, grid_mdagm;
+    int pc_tile;         // slices per run of the sliding-window preconditioner kernel (0 = generic kernel)
+    int pc_gx, pc_gy, n_part_rz;
     // CG chunk graph
     cudaGraphExec_t cg_graph;
     void *cg_graph_x;        // x pointer baked into the graph

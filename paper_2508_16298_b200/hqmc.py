@@ -25,7 +25,7 @@ SYMBOLS = [
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
     "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
-    "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
+    "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
 
 
@@ -122,6 +122,9 @@ class HQMC:
     def set_mdagm_kernel(self, which: int):
         """0 = streaming (TMA) kernel, 1 = register-only kernel."""
         _check(_lib.hqmc_set_mdagm_kernel(self._ctx, C.c_int(which)))
+
+    def set_precond_tile(self, slices_per_run: int):
+        _check(_lib.hqmc_set_precond_tile(self._ctx, C.c_int(slices_per_run)))
 
     # ---- operators ----------------------------------------------------------------------------
     def _apply(self, fn, v, out):

@@ -72,7 +72,7 @@ def test_config2_twenty_MdagM(hq):
     g.close()
 
 
-@pytest.mark.parametrize("L,Nt,W", [(4, 8, 6), (6, 10, 3), (12, 30, 6), (4, 8, 0)])
+@pytest.mark.parametrize("L,Nt,W", [(4, 8, 6), (6, 10, 3), (12, 30, 6), (4, 8, 0), (12, 41, 6), (14, 20, 1), (6, 40, 8)])
 def test_precond_and_taps(hq, L, Nt, W):
     o, g, theta = setup(hq, L, Nt, 3, W=W)
     if W > 0:
@@ -80,6 +80,9 @@ def test_precond_and_taps(hq, L, Nt, W):
     v = inputs.complex_gaussian((Nt, L, L), 7, inputs.STREAM_VEC)
     ref = o.precond(v) if W > 0 else v
     assert rel(g.precond(dev(v)).cpu().numpy(), ref) <= 1e-13
+    for tile in (1, 5, 16, 17, Nt):     # run lengths of the sliding-window kernel: shorter than, equal to and past its 16-slot ring
+        g.set_precond_tile(tile)
+        assert rel(g.precond(dev(v)).cpu().numpy(), ref) <= 1e-13, tile
     g.close()
 
 
