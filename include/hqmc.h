@@ -137,7 +137,8 @@ int hqmc_get_kernel_stats(hqmc_ctx *ctx, int which, long long *launches_out, dou
  * phases; default where its staging buffers fit shared memory, L <= 48 in complex128), 1 = register-only kernel. */
 int hqmc_set_time_tile(hqmc_ctx *ctx, int slices_per_cta);
 int hqmc_set_mdagm_kernel(hqmc_ctx *ctx, int which);
-/* Slices per run of the sliding-window preconditioner kernel (W = 1..6); 0 = library default. */
+/* Preconditioner kernel for W = 1..6: n > 0: TMA-tiled kernel, runs of n slices per CTA; n < 0: register-ring
+ * kernel with runs of -n slices; 0 = library default (TMA-tiled). */
 int hqmc_set_precond_tile(hqmc_ctx *ctx, int slices_per_run);
 
 const char *hqmc_strerror(int status);

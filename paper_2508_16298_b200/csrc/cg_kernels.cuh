@@ -6,6 +6,7 @@
 // in all CTAs, run-to-run deterministic, with no atomics, no extra kernel and no host round trip.
 #pragma once
 #include "kernels.cuh"
+#include "tma.cuh"
 
 namespace hqmc {
 

@@ -140,30 +140,42 @@ template <typename T> static int do_mdagm(hqmc_ctx *c, const void *in, void *out
     });
 }
 
-// choose the preconditioner kernel and its grid; fixes the number of <r,z> partials the CG kernels sum
+// choose the preconditioner kernel and its grid; fixes the number of <r,z> partials the CG kernels sum.
+// tile > 0: TMA-tiled kernel with runs of `tile` slices; tile < 0: register-ring kernel with runs of -tile; 0: default.
 static void precond_cfg(hqmc_ctx *c, int tile) {
     const int W = c->taps.W;
-    if (W < 1 || W > 6) { c->pc_tile = 0; c->pc_gx = c->grid_ew; c->pc_gy = 1; c->n_part_rz = c->grid_ew; return; }
+    c->pc_smem = 0;
+    if (W < 1 || W > 6) { c->pc_kind = 0; c->pc_tile = 0; c->pc_gx = c->grid_ew; c->pc_gy = 1; c->n_part_rz = c->grid_ew; return; }
     const int gx = (c->g.Vs + 127) / 128;
-    if (tile <= 0) {
-        int want = (4 * c->n_sm + gx - 1) / gx;                 // about 4 CTAs of 128 threads per SM
+    c->pc_kind = tile < 0 ? 1 : 2;
+    if (tile < 0) tile = -tile;
+    if (tile == 0) {
+        int want = (2 * c->n_sm + gx - 1) / gx;                 // about 2 CTAs of 128 threads (and <= 72 KB of tile) per SM
         tile = (c->g.Nt + want - 1) / want;
         if (tile < 24) tile = 24;                                // keep the 2W halo re-reads <= 50 %
     }
     if (tile > c->g.Nt) tile = c->g.Nt;
+    if (c->pc_kind == 2 && tile > 96) tile = 96;                 // tile rows (tile + 2W <= 108) x 128 sites x 16 B <= 216 KB
     while ((long long)gx * ((c->g.Nt + tile - 1) / tile) > HQMC_MAX_PART) ++tile;
+    if (c->pc_kind == 2 && tile > 96) c->pc_kind = 1;
     c->pc_tile = tile; c->pc_gx = gx; c->pc_gy = (c->g.Nt + tile - 1) / tile; c->n_part_rz = c->pc_gx * c->pc_gy;
+    if (c->pc_kind == 2) c->pc_smem = (size_t)(tile + 2 * W) * 128 * c->esz;
 }
 
 template <typename T, int W> static int launch_precond_win(hqmc_ctx *c, const void *in, void *out, double *part_rz, int mode) {
     typedef typename Cx<T>::type T2;
+    if (c->pc_kind == 2) {
+        CUDA_TRY(cudaFuncSetAttribute(k_precond_tma<T, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->pc_smem));
+        return launch(c, HQMC_K_PRECOND, k_precond_tma<T, W>, dim3(c->pc_gx, c->pc_gy), dim3(128), c->pc_smem, c->g, c->taps,
+                      (const T2 *)in, (T2 *)out, part_rz, (const double *)c->d_part_rr, c->grid_ew, c->d_state, mode, c->pc_tile);
+    }
     return launch(c, HQMC_K_PRECOND, k_precond_win<T, W>, dim3(c->pc_gx, c->pc_gy), dim3(128), 0, c->g, c->taps, (const T2 *)in,
                   (T2 *)out, part_rz, (const double *)c->d_part_rr, c->grid_ew, c->d_state, mode, c->pc_tile);
 }
 
 template <typename T> static int do_precond(hqmc_ctx *c, const void *in, void *out, double *part_rz, int mode) {
     typedef typename Cx<T>::type T2;
-    if (c->pc_tile > 0) {
+    if (c->pc_kind != 0) {
         switch (c->taps.W) {
             case 1: return launch_precond_win<T, 1>(c, in, out, part_rz, mode);
             case 2: return launch_precond_win<T, 2>(c, in, out, part_rz, mode);

@@ -231,7 +231,7 @@ extern "C" int hqmc_set_time_tile(hqmc_ctx *c, int tt) {
     return HQMC_OK;
 }
 extern "C" int hqmc_set_precond_tile(hqmc_ctx *c, int slices_per_run) {
-    if (!c || slices_per_run < 0) return HQMC_EINVAL;
+    if (!c) return HQMC_EINVAL;
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     precond_cfg(c, slices_per_run);
     return HQMC_OK;

@@ -14,6 +14,7 @@
 #include "force_kernels.cuh"
 #include "kernels.cuh"
 #include "mdagm_stream.cuh"
+#include "precond_tma.cuh"
 
 namespace hqmc {
 
@@ -72,6 +73,8 @@ struct hqmc_ctx {
     int grid_ew, grid_mdagm;
     int pc_tile;         // slices per run of the sliding-window preconditioner kernel (0 = generic kernel)
     int pc_gx, pc_gy, n_part_rz;
+    int pc_kind;         // 0: generic k_precond, 1: register-ring k_precond_win, 2: TMA-tiled k_precond_tma
+    size_t pc_smem;
     // CG chunk graph
     cudaGraphExec_t cg_graph;
     void *cg_graph_x;        // x pointer baked into the graph

@@ -15,6 +15,7 @@
 #include <cstdint>
 
 #include "kernels.cuh"
+#include "tma.cuh"
 
 namespace hqmc {
 
@@ -95,40 +96,6 @@ __global__ void k_phase_pack(Geo g, const double *__restrict__ theta, typename P
         packed[t * per + packed_slot(g, mu, y, x)] = PhasePack<T>::pack(theta[i], sc);
     }
 }
-
-// ------------------------------------------------------------------------------------------------
-// mbarrier / TMA bulk-copy helpers (PTX; SASS: SYNCS.*, UBLKCP)
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
-                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void bulk_s2g(void *dst_gmem, const void *src_smem, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------------
 // Lean single-block-per-thread engine for the streaming kernel: everything a thread needs is a handful of
@@ -249,7 +216,6 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
                         const double2 *__restrict__ tab_g, const typename Cx<T>::type *__restrict__ in,
                         typename Cx<T>::type *__restrict__ out, T C, double *__restrict__ part, const CgState *__restrict__ st) {
     typedef typename Cx<T>::type T2;
-    if (st != nullptr && *(volatile const int *)&st->done) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int nbp = blockDim.x;
     const StreamSmem<T> lay(g.Vs, nbp);
@@ -281,8 +247,14 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
         bulk_load(smem_raw + lay.vbuf, in_b + (size_t)tp * vbytes, vbytes, bar_v);
         bulk_load(pbuf, pk_b + (size_t)tp * pbytes, pbytes, bar_p);
     }
+    // The CG "done" flag is read only now, with the first slice already in flight (its latency is hidden).
+    const int done = (st != nullptr) ? *(volatile const int *)&st->done : 0;
     __syncthreads();                      // barrier inits visible to every thread
     if (sizeof(T) == 8) mbar_wait(bar_t, 0);
+    if (done) {                           // drain the copies aimed at this CTA's shared memory, then leave
+        mbar_wait(bar_v, 0); mbar_wait(bar_p, 0);
+        return;
+    }
 
     T2 w0, w1, w2, w3;                    // w_t
     LeanPh<T2> P;

@@ -80,7 +80,7 @@ def test_precond_and_taps(hq, L, Nt, W):
     v = inputs.complex_gaussian((Nt, L, L), 7, inputs.STREAM_VEC)
     ref = o.precond(v) if W > 0 else v
     assert rel(g.precond(dev(v)).cpu().numpy(), ref) <= 1e-13
-    for tile in (1, 5, 16, 17, Nt):     # run lengths of the sliding-window kernel: shorter than, equal to and past its 16-slot ring
+    for tile in (1, 5, 13, 16, 17, Nt, -1, -5, -16, -17, -Nt):   # TMA-tiled (>0) and register-ring (<0) kernels; runs shorter than, equal to and past the ring
         g.set_precond_tile(tile)
         assert rel(g.precond(dev(v)).cpu().numpy(), ref) <= 1e-13, tile
     g.close()
