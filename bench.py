@@ -35,6 +35,9 @@ METRIC = "MdagM_Gsite_per_s"
 UNIT = "Gsite/s"
 # algorithmic bytes per site (complex128): read v (16) + 2 link phases as theta (16) + write (16)
 BYTES_PER_SITE = {"mdagm": 48.0, "cg_axpy": 96.0, "precond": 32.0, "cg_dupdate": 48.0}
+# fused PCG vector kernels (default): "precond" class = k_cg_rz (read r, Od; write r', z), "cg_dupdate" class = k_cg_xd
+# (read x, d, z; write x, d)
+BYTES_PER_SITE_FUSED = {"mdagm": 48.0, "precond": 64.0, "cg_dupdate": 80.0}
 BYTES_PER_SITE_C64 = {k: v / 2 for k, v in BYTES_PER_SITE.items()}
 
 
@@ -271,7 +274,10 @@ def run_gpu(args):
     value = total_apps * N / (ms * 1e-3) / 1e9
     e2e_value = total_e2e_apps * N / e2e_s / 1e9
     peak, peak_src = measured_peaks()
-    bps = BYTES_PER_SITE if prec == "c128" else BYTES_PER_SITE_C64
+    fused = not kern.get("cg_axpy", (0, 0))[0]
+    bps = dict(BYTES_PER_SITE_FUSED if fused else BYTES_PER_SITE)
+    if prec != "c128":
+        bps = {k: v / 2 for k, v in bps.items()}
     per_kernel = {}
     for name, (n, kms) in kern.items():
         if n:

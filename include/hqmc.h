@@ -134,12 +134,19 @@ int hqmc_reset_stats(hqmc_ctx *ctx);
 int hqmc_get_kernel_stats(hqmc_ctx *ctx, int which, long long *launches_out, double *ms_out);
 /* Tuning knobs.  hqmc_set_time_tile: slices per CTA of the fused M^+M kernel (0 = library default: one CTA per SM
  * with the slices dealt out evenly).  hqmc_set_mdagm_kernel: 0 = streaming kernel (TMA bulk copies, packed link
- * phases; default where its staging buffers fit shared memory, L <= 48 in complex128), 1 = register-only kernel. */
+ * phases), 1 = register-only kernel, 2 = warp-specialised strip-decoupled streaming kernel (default where its
+ * staging buffers fit shared memory: L <= 48 in complex128). */
 int hqmc_set_time_tile(hqmc_ctx *ctx, int slices_per_cta);
 int hqmc_set_mdagm_kernel(hqmc_ctx *ctx, int which);
 /* Preconditioner kernel for W = 1..6: n > 0: TMA-tiled kernel, runs of n slices per CTA; n < 0: register-ring
  * kernel with runs of -n slices; 0 = library default (TMA-tiled). */
 int hqmc_set_precond_tile(hqmc_ctx *ctx, int slices_per_run);
+/* PCG vector kernels: 1 (default) = fused residual-update + preconditioner and fused x/d update where the
+ * TMA-tiled preconditioner applies (3 kernels per iteration); 0 = the four separate kernels. */
+int hqmc_set_cg_fusion(hqmc_ctx *ctx, int on);
+/* TIMING ONLY: bit k of mask set = kernels of class HQMC_K_<k> are not launched (leave-one-out timing of a kernel
+ * inside the graph-replayed PCG iteration; the numerical results are then meaningless).  0 restores normal operation. */
+int hqmc_set_debug_skip(hqmc_ctx *ctx, unsigned mask);
 
 const char *hqmc_strerror(int status);
 const char *hqmc_last_error(void); /* text of the last CUDA error seen by this thread, or "" */

@@ -172,15 +172,32 @@ __device__ __forceinline__ double block_sum(double v, double *red) {
     }
     return r;
 }
+// Lane-strided sum of n partials in a fixed order (16 independent loads in flight per lane, so a few hundred
+// partials cost one or two L2 round trips instead of one per element), then the shuffle tree; all 32 lanes of the
+// calling warp get the result.
+__device__ __forceinline__ double sum_partials_lanes(const double *__restrict__ part, int n, int lane) {
+    double s = 0.0;
+    int i = lane;
+    for (; i + 15 * 32 < n; i += 16 * 32) {
+        double a[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) a[k] = part[i + 32 * k];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) s += a[k];
+    }
+    {
+        double a[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) a[k] = (i + 32 * k < n) ? part[i + 32 * k] : 0.0;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) s += a[k];
+    }
+    s = warp_sum(s);
+    return __shfl_sync(0xffffffffu, s, 0);
+}
 // Sum n partials in a fixed order; every thread of the FIRST WARP gets the result (others get 0).
 __device__ __forceinline__ double sum_partials_warp0(const double *__restrict__ part, int n) {
-    double s = 0.0;
-    if (threadIdx.x < 32) {
-        for (int i = threadIdx.x; i < n; i += 32) s += part[i];
-        s = warp_sum(s);
-        s = __shfl_sync(0xffffffffu, s, 0);
-    }
-    return s;
+    return (threadIdx.x < 32) ? sum_partials_lanes(part, n, threadIdx.x) : 0.0;
 }
 
 }  // namespace hqmc

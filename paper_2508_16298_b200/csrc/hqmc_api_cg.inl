@@ -7,9 +7,18 @@
 // into a no-op after convergence, so tolerance-based stopping and graph replay coexist.  The host looks
 // at the flag once per chunk.
 
+// Fused form (W = 1..6): [O d + <d,Od>] [r' = r - alpha Od, z = P r', ||r'||^2, <r',z>] [x += alpha d, d = z + beta d,
+// bookkeeping] -- 3 kernels, r ping-pongs between two buffers (iteration parity = `par`).
 template <typename T> static int cg_iteration(hqmc_ctx *c, void *x, int par) {
     typedef typename Cx<T>::type T2;
     HQ_TRY(do_mdagm<T>(c, c->d_d, c->d_Od, true, c->d_state));
+    if (c->cg_fused) {
+        void *rin = par ? c->d_r2 : c->d_r, *rout = par ? c->d_r : c->d_r2;
+        HQ_TRY(do_cg_rz<T>(c, rin, rout, (const double *)c->d_part_rz[par], c->d_part_rz[par ^ 1]));
+        return launch(c, HQMC_K_DUPDATE, k_cg_xd<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_d, (const T2 *)c->d_z,
+                      (const double *)c->d_part_rz[par], (const double *)c->d_part_rz[par ^ 1], c->n_part_f,
+                      (const double *)c->d_part_dOd, c->grid_mdagm, (const double *)c->d_part_rr, c->d_state);
+    }
     HQ_TRY(launch(c, HQMC_K_AXPY, k_cg_axpy<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_r, (const T2 *)c->d_d,
                   (const T2 *)c->d_Od, (const double *)c->d_part_rz[par], c->n_part_rz, (const double *)c->d_part_dOd,
                   c->grid_mdagm, c->d_part_rr, (const CgState *)c->d_state));
@@ -21,7 +30,7 @@ template <typename T> static int cg_iteration(hqmc_ctx *c, void *x, int par) {
 }
 
 template <typename T> static int cg_build_graph(hqmc_ctx *c, void *x) {
-    if (c->cg_graph && c->cg_graph_x == x && c->cg_graph_tile == c->time_tile) return HQMC_OK;
+    if (c->cg_graph && c->cg_graph_x == x && c->cg_graph_tile == c->time_tile && c->cg_graph_fused == c->cg_fused) return HQMC_OK;
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     for (int i = 0; i < HQMC_K_COUNT; ++i) c->graph_nodes[i] = 0;
     cudaGraph_t graph = nullptr;
@@ -38,6 +47,7 @@ template <typename T> static int cg_build_graph(hqmc_ctx *c, void *x) {
     CUDA_TRY(e);
     c->cg_graph_x = x;
     c->cg_graph_tile = c->time_tile;
+    c->cg_graph_fused = c->cg_fused;
     return HQMC_OK;
 }
 
@@ -49,6 +59,8 @@ template <typename T> static int cg_solve_t(hqmc_ctx *c, const void *rhs, void *
     c->h_state->iters = 0; c->h_state->max_iter = max_iter; c->h_state->done = 0; c->h_state->pad = 0;
     CUDA_TRY(cudaMemcpyAsync(c->d_state, c->h_state, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
     // x_0 = 0, r_0 = rhs, z_0 = P r_0, d_0 = z_0
+    if (c->cg_fused)   // the fused kernels sum n_part_f >= n_part_rz partials: the start-up kernel fills the first n_part_rz
+        CUDA_TRY(cudaMemsetAsync(c->d_part_rz[0], 0, sizeof(double) * HQMC_MAX_PART, c->stream));
     HQ_TRY(launch(c, HQMC_K_MISC, k_cg_init<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (const T2 *)rhs, (T2 *)x, (T2 *)c->d_r,
                   c->d_part_rr));
     HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[0], 1));

@@ -64,8 +64,8 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     c->esz = (prm->prec == HQMC_C128) ? 16 : 8;
     c->own_stream = (cuda_stream == nullptr);
     c->stream = (cudaStream_t)cuda_stream;
-    c->cg_graph = nullptr; c->cg_graph_x = nullptr; c->cg_graph_tile = 0; c->cg_chunk = 32;
-    c->profiling = false; c->capturing = false; c->theta_set = false;
+    c->cg_graph = nullptr; c->cg_graph_x = nullptr; c->cg_graph_tile = 0; c->cg_graph_fused = false; c->cg_chunk = 32;
+    c->profiling = false; c->capturing = false; c->theta_set = false; c->fused_allowed = true; c->cg_fused = false; c->skip_mask = 0;
     for (int i = 0; i < HQMC_K_COUNT; ++i) { c->launches[i] = 0; c->graph_nodes[i] = 0; c->ms[i] = 0.0; }
     int st = HQMC_OK;
     auto fail = [&](int s) { hqmc_destroy(c); return s; };
@@ -100,6 +100,11 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
         c->stream_smem = need;
         c->use_stream = (c->cfg.bpt == 1) && need <= (size_t)prop.sharedMemPerBlockOptin && (size_t)c->g.Vs * 16 < (1u << 20);
         c->stream_on = c->use_stream;
+        const int ws_ns = ws_geometry(h, c->cfg.threads).ns;
+        c->ws_smem = (prm->prec == HQMC_C128) ? WsSmem<double>(c->g.Vs, c->cfg.threads, h, ws_ns).total
+                                              : WsSmem<float>(c->g.Vs, c->cfg.threads, h, ws_ns).total;
+        c->use_ws = c->use_stream && c->cfg.threads + 32 <= 608 && c->ws_smem <= (size_t)prop.sharedMemPerBlockOptin;
+        c->ws_on = false;   // measured slower than k_mdagm_stream (profiles/): kept selectable
     }
     if (c->use_stream) {
         ALLOC(c->d_packed, 2 * c->N * 8);
@@ -113,7 +118,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
         cudaError_t e = cudaMemcpy(c->d_tab, tab.data(), sizeof(double2) * tab.size(), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) { g_last_error = cudaGetErrorString(e); return fail(HQMC_ECUDA); }
     }
-    ALLOC(c->d_r, vb); ALLOC(c->d_z, vb); ALLOC(c->d_d, vb); ALLOC(c->d_Od, vb); ALLOC(c->d_X, vb); ALLOC(c->d_phi, vb);
+    ALLOC(c->d_r, vb); ALLOC(c->d_r2, vb); ALLOC(c->d_z, vb); ALLOC(c->d_d, vb); ALLOC(c->d_Od, vb); ALLOC(c->d_X, vb); ALLOC(c->d_phi, vb);
     ALLOC(c->d_p, tb); ALLOC(c->d_force, tb);
     ALLOC(c->d_part_dOd, sizeof(double) * HQMC_MAX_PART); ALLOC(c->d_part_rr, sizeof(double) * HQMC_MAX_PART);
     ALLOC(c->d_part_rz[0], sizeof(double) * HQMC_MAX_PART); ALLOC(c->d_part_rz[1], sizeof(double) * HQMC_MAX_PART);
@@ -141,7 +146,7 @@ extern "C" int hqmc_destroy(hqmc_ctx *c) {
     if (c->cg_graph) cudaGraphExecDestroy(c->cg_graph);
     for (auto &ep : c->pending) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (auto &ep : c->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-    void *ptrs[] = {c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
+    void *ptrs[] = {c->d_r2, c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
                     c->d_part_rr, c->d_part_rz[0], c->d_part_rz[1], c->d_part_misc, c->d_state, c->d_scal};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (c->h_state) cudaFreeHost(c->h_state);
@@ -236,10 +241,24 @@ extern "C" int hqmc_set_precond_tile(hqmc_ctx *c, int slices_per_run) {
     precond_cfg(c, slices_per_run);
     return HQMC_OK;
 }
+extern "C" int hqmc_set_debug_skip(hqmc_ctx *c, unsigned mask) {
+    if (!c) return HQMC_EINVAL;
+    c->skip_mask = mask;
+    if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+    return HQMC_OK;
+}
+extern "C" int hqmc_set_cg_fusion(hqmc_ctx *c, int on) {
+    if (!c) return HQMC_EINVAL;
+    c->fused_allowed = on != 0;
+    if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+    precond_cfg(c, c->pc_kind == 1 ? -c->pc_tile : c->pc_tile);
+    return HQMC_OK;
+}
 extern "C" int hqmc_set_mdagm_kernel(hqmc_ctx *c, int which) {
-    if (!c || which < 0 || which > 1) return HQMC_EINVAL;
-    if (which == 0 && !c->use_stream) return HQMC_EINVAL;
-    c->stream_on = (which == 0);
+    if (!c || which < 0 || which > 2) return HQMC_EINVAL;
+    if ((which == 0 && !c->use_stream) || (which == 2 && !c->use_ws)) return HQMC_EINVAL;
+    c->stream_on = (which != 1);
+    c->ws_on = (which == 2);
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     return hqmc_set_time_tile(c, 0);
 }

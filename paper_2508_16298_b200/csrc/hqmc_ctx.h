@@ -14,6 +14,7 @@
 #include "force_kernels.cuh"
 #include "kernels.cuh"
 #include "mdagm_stream.cuh"
+#include "mdagm_ws.cuh"
 #include "precond_tma.cuh"
 
 namespace hqmc {
@@ -58,7 +59,9 @@ struct hqmc_ctx {
     void *d_ph;          // phase table [Nt][2][L][L] complex
     void *d_packed;      // packed link phases [Nt][4][nb][2] (8 B each) for the streaming M^+M kernel
     double2 *d_tab;      // [2][1024] tanh(a) e^{i k delta} (half step, full step)
-    bool stream_on;      // runtime switch (hqmc_set_mdagm_kernel)
+    bool stream_on;      // runtime switch (hqmc_set_mdagm_kernel): a streaming kernel is selected
+    bool use_ws, ws_on;  // warp-specialised strip kernel usable / selected
+    size_t ws_smem;
     bool use_stream;     // streaming kernel usable (BPT == 1 and its shared memory fits)
     size_t stream_smem;
     void *d_r, *d_z, *d_d, *d_Od, *d_X, *d_phi;   // CG vectors, trajectory solution / pseudofermion
@@ -73,14 +76,20 @@ struct hqmc_ctx {
     int grid_ew, grid_mdagm;
     int pc_tile;         // slices per run of the sliding-window preconditioner kernel (0 = generic kernel)
     int pc_gx, pc_gy, n_part_rz;
+    bool fused_allowed;  // knob (hqmc_set_cg_fusion)
+    bool cg_fused;       // PCG runs on the fused k_cg_rz / k_cg_xd kernels (pc_kind == 2)
+    int f_gx, f_gy, n_part_f; size_t f_smem;
+    void *d_r2;          // second residual buffer (k_cg_rz writes r' out of place)
     int pc_kind;         // 0: generic k_precond, 1: register-ring k_precond_win, 2: TMA-tiled k_precond_tma
     size_t pc_smem;
     // CG chunk graph
     cudaGraphExec_t cg_graph;
     void *cg_graph_x;        // x pointer baked into the graph
     int cg_graph_tile;
+    bool cg_graph_fused;
     int cg_chunk;            // iterations per graph launch
     // instrumentation
+    unsigned skip_mask;   // timing-only: kernel classes NOT launched inside the PCG iteration (hqmc_set_debug_skip)
     bool profiling;
     bool capturing;
     long long launches[HQMC_K_COUNT];

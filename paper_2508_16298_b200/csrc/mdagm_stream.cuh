@@ -185,12 +185,13 @@ __device__ __forceinline__ void lean_load_phases(const unsigned char *pbuf, cons
 
 template <typename T> struct StreamSmem {
     // byte offsets inside dynamic shared memory (nbp = threads per CTA >= nb)
-    size_t tab, vbuf, pbuf, obuf, exch, red, bars, total;
+    size_t tab, vbuf, vbuf2, pbuf, obuf, exch, red, bars, total;
     __host__ __device__ StreamSmem(int Vs, int nbp) {
         typedef typename Cx<T>::type T2;
         size_t o = 0;
         tab = o;  o += (sizeof(T) == 8) ? (size_t)2 * HQMC_PHASE_K * sizeof(double2) : 0;
         vbuf = o; o += (size_t)Vs * sizeof(T2);
+        vbuf2 = o; o += (size_t)Vs * sizeof(T2);
         pbuf = o; o += (size_t)2 * Vs * 8;
         obuf = o; o += (size_t)Vs * sizeof(T2);
         exch = o; o += (size_t)4 * nbp * sizeof(T2);
@@ -221,11 +222,11 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
     const StreamSmem<T> lay(g.Vs, nbp);
     const double2 *tab = reinterpret_cast<const double2 *>(smem_raw + lay.tab);
     unsigned char *pbuf = smem_raw + lay.pbuf;
-    const T2 *vsm = reinterpret_cast<const T2 *>(smem_raw + lay.vbuf);
+    const T2 *vsA = reinterpret_cast<const T2 *>(smem_raw + lay.vbuf), *vsB = reinterpret_cast<const T2 *>(smem_raw + lay.vbuf2);
     T2 *osm = reinterpret_cast<T2 *>(smem_raw + lay.obuf);
     T2 *ex = reinterpret_cast<T2 *>(smem_raw + lay.exch);
     double *red = reinterpret_cast<double *>(smem_raw + lay.red);
-    uint64_t *bar_v = reinterpret_cast<uint64_t *>(smem_raw + lay.bars), *bar_p = bar_v + 1, *bar_t = bar_v + 2;
+    uint64_t *bar_v = reinterpret_cast<uint64_t *>(smem_raw + lay.bars), *bar_p = bar_v + 1, *bar_t = bar_v + 2, *bar_v2 = bar_v + 3;
     LeanIdx b;
     make_lean(g, threadIdx.x, b);
 
@@ -237,22 +238,27 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
     const unsigned char *pk_b = reinterpret_cast<const unsigned char *>(packed);
     unsigned char *out_b = reinterpret_cast<unsigned char *>(out);
     const bool leader = threadIdx.x == 0;
-    uint32_t par_v = 0, par_p = 0;
+    uint32_t par_vA = 0, par_vB = 0, par_p = 0;
     const int tp = (t0 == 0) ? g.Nt - 1 : t0 - 1;
+    const int nsl = t1 - t0;
+    auto wrap = [&](int t) { return t >= g.Nt ? t - g.Nt : t; };
 
+    // v is kept TWO slices deep (buffers A, B alternate), the links one slice deep: every copy is issued a full
+    // slice of compute before it is needed, so HBM stays busy while the sweeps run.
     if (leader) {
-        mbar_init(bar_v, 1); mbar_init(bar_p, 1); mbar_init(bar_t, 1);
+        mbar_init(bar_v, 1); mbar_init(bar_v2, 1); mbar_init(bar_p, 1); mbar_init(bar_t, 1);
         mbar_fence_init();
         if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_K * sizeof(double2), bar_t);
         bulk_load(smem_raw + lay.vbuf, in_b + (size_t)tp * vbytes, vbytes, bar_v);
         bulk_load(pbuf, pk_b + (size_t)tp * pbytes, pbytes, bar_p);
+        bulk_load(smem_raw + lay.vbuf2, in_b + (size_t)t0 * vbytes, vbytes, bar_v2);
     }
-    // The CG "done" flag is read only now, with the first slice already in flight (its latency is hidden).
+    // The CG "done" flag is read only now, with the first slices already in flight (its latency is hidden).
     const int done = (st != nullptr) ? *(volatile const int *)&st->done : 0;
     __syncthreads();                      // barrier inits visible to every thread
     if (sizeof(T) == 8) mbar_wait(bar_t, 0);
     if (done) {                           // drain the copies aimed at this CTA's shared memory, then leave
-        mbar_wait(bar_v, 0); mbar_wait(bar_p, 0);
+        mbar_wait(bar_v, 0); mbar_wait(bar_v2, 0); mbar_wait(bar_p, 0);
         return;
     }
 
@@ -261,43 +267,48 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
     double acc = 0.0;
 
     // ---- prologue: w_{t0} = v_{t0} - sigma_{tp} C B_{tp} v_{tp}
-    mbar_wait(bar_v, par_v); par_v ^= 1;
+    mbar_wait(bar_v, par_vA); par_vA ^= 1;
     mbar_wait(bar_p, par_p); par_p ^= 1;
-    w0 = vsm[b.o0]; w1 = vsm[b.o1]; w2 = vsm[b.o2]; w3 = vsm[b.o3];
+    w0 = vsA[b.o0]; w1 = vsA[b.o1]; w2 = vsA[b.o2]; w3 = vsA[b.o3];
     lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
     lean_apply_B(ex, nbp, b, P, w0, w1, w2, w3, [&]() {
-        if (leader) {
-            bulk_load(smem_raw + lay.vbuf, in_b + (size_t)t0 * vbytes, vbytes, bar_v);
+        if (leader) {                     // buffer A and pbuf have been read by everyone
+            bulk_load(smem_raw + lay.vbuf, in_b + (size_t)wrap(t0 + 1) * vbytes, vbytes, bar_v);
             bulk_load(pbuf, pk_b + (size_t)t0 * pbytes, pbytes, bar_p);
         }
     });
     {
         const T sC = (tp == g.Nt - 1) ? C : -C;
-        mbar_wait(bar_v, par_v); par_v ^= 1;
+        mbar_wait(bar_v2, par_vB); par_vB ^= 1;
         mbar_wait(bar_p, par_p); par_p ^= 1;
-        T2 v0 = vsm[b.o0], v1 = vsm[b.o1], v2 = vsm[b.o2], v3 = vsm[b.o3];
+        T2 v0 = vsB[b.o0], v1 = vsB[b.o1], v2 = vsB[b.o2], v3 = vsB[b.o3];
         w0.x = fma(sC, w0.x, v0.x); w0.y = fma(sC, w0.y, v0.y); w1.x = fma(sC, w1.x, v1.x); w1.y = fma(sC, w1.y, v1.y);
         w2.x = fma(sC, w2.x, v2.x); w2.y = fma(sC, w2.y, v2.y); w3.x = fma(sC, w3.x, v3.x); w3.y = fma(sC, w3.y, v3.y);
         lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
     }
 
-    for (int t = t0; t < t1; ++t) {
-        const int tn = (t + 1 == g.Nt) ? 0 : t + 1;
+    for (int i = 0; i < nsl; ++i) {
+        const int t = t0 + i;
+        const int tn = wrap(t + 1);
         const T sC = (t == g.Nt - 1) ? C : -C;
-        const bool more = (t + 1 < t1);
-        // v = B_t v_t / C; v_t is still in vbuf (it is refilled only after the first barrier below, by which time
-        // everyone has read it and pbuf) and obuf holds out_{t-1} completely: thread 0 stores it and fetches v_{t+1}
-        // and the phases of slice t+1.
-        T2 v0 = vsm[b.o0], v1 = vsm[b.o1], v2 = vsm[b.o2], v3 = vsm[b.o3];
+        const bool more = (i + 1 < nsl);
+        const bool odd = i & 1;
+        const T2 *vcur = odd ? vsA : vsB, *vnxt = odd ? vsB : vsA;       // v_t sits in buffer (i+1)&1, v_{t+1} in buffer i&1
+        // v = B_t v_t / C.  After the first barrier of the sweep sequence everyone has read v_t and (at the end of the
+        // previous iteration) the links, and obuf holds out_{t-1} completely: thread 0 stores it and fetches v_{t+2}
+        // into the buffer v_t occupied and the links of slice t+1.
+        T2 v0 = vcur[b.o0], v1 = vcur[b.o1], v2 = vcur[b.o2], v3 = vcur[b.o3];
         lean_apply_B(ex, nbp, b, P, v0, v1, v2, v3, [&]() {
             if (leader) {
-                if (t > t0) { bulk_s2g(out_b + (size_t)(t - 1) * vbytes, osm, vbytes); bulk_commit(); }
-                bulk_load(smem_raw + lay.vbuf, in_b + (size_t)tn * vbytes, vbytes, bar_v);
-                if (more) bulk_load(pbuf, pk_b + (size_t)tn * pbytes, pbytes, bar_p);
+                if (i > 0) { bulk_s2g(out_b + (size_t)(t - 1) * vbytes, osm, vbytes); bulk_commit(); }
+                if (more) {
+                    bulk_load(smem_raw + (odd ? lay.vbuf : lay.vbuf2), in_b + (size_t)wrap(t + 2) * vbytes, vbytes, odd ? bar_v : bar_v2);
+                    bulk_load(pbuf, pk_b + (size_t)tn * pbytes, pbytes, bar_p);
+                }
             }
         });
-        mbar_wait(bar_v, par_v); par_v ^= 1;
-        T2 n0 = vsm[b.o0], n1 = vsm[b.o1], n2 = vsm[b.o2], n3 = vsm[b.o3];       // v_{t+1}
+        if (odd) { mbar_wait(bar_v2, par_vB); par_vB ^= 1; } else { mbar_wait(bar_v, par_vA); par_vA ^= 1; }
+        T2 n0 = vnxt[b.o0], n1 = vnxt[b.o1], n2 = vnxt[b.o2], n3 = vnxt[b.o3];   // v_{t+1}
         T2 q0, q1, q2, q3;                                                         // w_{t+1}, then B_t w_{t+1}
         q0.x = fma(sC, v0.x, n0.x); q0.y = fma(sC, v0.y, n0.y); q1.x = fma(sC, v1.x, n1.x); q1.y = fma(sC, v1.y, n1.y);
         q2.x = fma(sC, v2.x, n2.x); q2.y = fma(sC, v2.y, n2.y); q3.x = fma(sC, v3.x, n3.x); q3.y = fma(sC, v3.y, n3.y);

@@ -47,11 +47,11 @@ def test_M_Mdag_MdagM(hq, L, Nt, seed):
     assert rel(g.apply_Mdag(dv).cpu().numpy(), o.apply_Mdag(theta, v)) <= 1e-12
     ref = o.apply_MdagM(theta, v)
     assert rel(g.apply_MdagM(dv).cpu().numpy(), ref) <= 1e-12
-    for which in (0, 1):              # 0: streaming (TMA) kernel where it fits shared memory, 1: register-only kernel
+    for which in (2, 0, 1):           # 2: warp-specialised strips, 0: streaming (TMA) kernel (both where they fit), 1: register-only
         try:
             g.set_mdagm_kernel(which)
         except hq.HqmcError:
-            assert which == 0 and L > 48
+            assert which in (0, 2) and L > 48
             continue
         for tt in (0, 1, 2, 3, Nt):   # default split and every time-tile shape incl. ragged last tile and one-CTA-for-all
             g.set_time_tile(tt)
@@ -113,6 +113,26 @@ def test_cg_solution_and_iterations(hq, L, Nt, seed, W):
     xf, itf, relf, _ = g.cg_solve(dev(phi), 0.0, 11)
     xo, ito, relo = o.pcg(theta, phi, 0.0, 11)
     assert itf == ito == 11 and rel(xf.cpu().numpy(), xo) <= 1e-11 and abs(relf - relo) <= 1e-9 * relo
+    g.close()
+
+
+@pytest.mark.parametrize("L,Nt,seed,W", [(8, 40, 2, 6), (12, 30, 3, 3), (6, 10, 1, 1)])
+def test_cg_fused_and_unfused_kernels_agree_with_oracle(hq, L, Nt, seed, W):
+    """The 3-kernel fused iteration (k_cg_rz + k_cg_xd, default) and the 4-kernel one give the oracle's iterates."""
+    o, g, theta = setup(hq, L, Nt, seed, W=W)
+    eta = inputs.complex_gaussian((Nt, L, L), seed)
+    phi = o.apply_Mdag(theta, eta)
+    xo, ito, relo = o.pcg(theta, phi, 0.0, 25)
+    x_ref, it_ref, _ = o.pcg(theta, phi, 1e-10, 100000)
+    for fused in (True, False):
+        g.set_cg_fusion(fused)
+        for tile in (0, 7):
+            g.set_precond_tile(tile)
+            xf, itf, relf, _ = g.cg_solve(dev(phi), 0.0, 25)           # fixed count: same iterate, same residual
+            assert itf == 25 and rel(xf.cpu().numpy(), xo) <= 1e-11 and abs(relf - relo) <= 1e-9 * relo, (fused, tile)
+            x, it, relres, ok = g.cg_solve(dev(phi), 1e-10, 100000)
+            assert ok and relres <= 1e-10 and abs(it - it_ref) <= max(2, it_ref // 100), (fused, tile)
+            assert rel(x.cpu().numpy(), x_ref) <= 1e-9, (fused, tile)
     g.close()
 
 
