@@ -38,7 +38,8 @@ BYTES_PER_SITE = {"mdagm": 48.0, "cg_axpy": 96.0, "precond": 32.0, "cg_dupdate":
 # fused PCG vector kernels (default): "precond" class = k_cg_rz (read r, Od; write r', z), "cg_dupdate" class = k_cg_xd
 # (read x, d, z; write x, d)
 BYTES_PER_SITE_FUSED = {"mdagm": 48.0, "precond": 64.0, "cg_dupdate": 80.0}
-BYTES_PER_SITE_C64 = {k: v / 2 for k, v in BYTES_PER_SITE.items()}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/), L=48, c128
+TRAFFIC_NCU = {"mdagm": 35.6e6}
 
 
 def measured_peaks():
@@ -244,17 +245,13 @@ def run_gpu(args):
     vb, tb = N * (16 if prec == "c128" else 8), 2 * N * 8
     h2d, d2h = (tb + vb) + (2 * tb + vb), vb + 2 * tb
 
-    # ---- per-kernel timing of the same step (library-side CUDA events on the launching stream, no graph replay)
+    # ---- per-kernel cost INSIDE the graph-replayed PCG iteration, by leave-one-out: the same fixed-count solve is timed
+    # (CUDA events on the library's stream) with all kernels and with one kernel class not launched; the difference is
+    # that kernel's cost in the launch configuration the step uses.  The class that carries the iteration bookkeeping
+    # cannot be left out: it gets the remainder.  (Per-launch events would add the launch gaps of a non-replayed run.)
     kern = None
     if rank == 0:
-        g.set_profiling(True)
-        step_device(); torch.cuda.synchronize()
-        g.reset_stats()
-        for _ in range(max(1, min(3, args.steps))):
-            step_device()
-        torch.cuda.synchronize()
-        kern = g.kernel_stats()
-        g.set_profiling(False)
+        kern = pcg_kernel_costs(g, torch, d_phi, I)
 
     # ---- M^+M kernel alone, cold (rotating 8 buffer pairs > L2) and warm (same buffers)
     sweep = None
@@ -274,28 +271,21 @@ def run_gpu(args):
     value = total_apps * N / (ms * 1e-3) / 1e9
     e2e_value = total_e2e_apps * N / e2e_s / 1e9
     peak, peak_src = measured_peaks()
-    fused = not kern.get("cg_axpy", (0, 0))[0]
+    fused = "cg_axpy" not in kern["us"]
     bps = dict(BYTES_PER_SITE_FUSED if fused else BYTES_PER_SITE)
     if prec != "c128":
         bps = {k: v / 2 for k, v in bps.items()}
     per_kernel = {}
-    for name, (n, kms) in kern.items():
-        if n:
-            per_kernel[name] = {"launches": n, "avg_us": 1e3 * kms / n, "total_ms": kms}
-            if name in bps:
-                per_kernel[name]["alg_GBps"] = bps[name] * N / (1e-3 * kms / n) / 1e9
-    tot_k = sum(v["total_ms"] for v in per_kernel.values())
-    for v in per_kernel.values():
-        v["share"] = v["total_ms"] / tot_k
-    dom = max((k for k in per_kernel if k in bps), key=lambda k: per_kernel[k]["total_ms"])
+    for name, us in kern["us"].items():
+        per_kernel[name] = {"us_in_graph": us, "share_of_iteration": us / kern["iter_us"],
+                            "alg_bytes_per_site": bps[name], "alg_GBps": bps[name] * N / us / 1e3}
+    dom = max(per_kernel, key=lambda k: per_kernel[k]["us_in_graph"])
     achieved = per_kernel[dom]["alg_GBps"]
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "alg_bytes_per_site": bps[dom],
-                "how": "library CUDA events around every launch of the kernel on its stream during the same step (no graph replay)"}
+                "traffic": TRAFFIC_NCU.get(dom), "peak_source": peak_src, "alg_bytes_per_site": bps[dom],
+                "how": "leave-one-out CUDA-event timing of the graph-replayed fixed-count PCG solve (bench.py pcg_kernel_costs)"}
     ms_per_step = ms / args.steps
-    # fixed-count PCG iteration cost inside the timed region (graph replay): all four kernels of an iteration
-    cg_share = sum(per_kernel[k]["total_ms"] for k in ("mdagm", "cg_axpy", "precond", "cg_dupdate") if k in per_kernel) / tot_k
-    us_per_iter = 1e3 * ms_per_step * cg_share / (2 * I)
+    us_per_iter = kern["iter_us"]
     cb_dt, cb_apps, cb_threads = oracle_step_sample(L, Ntau, c["seed"], args.ref_cg_iters)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -314,6 +304,36 @@ def run_gpu(args):
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def pcg_kernel_costs(g, torch, d_phi, iters):
+    """-> {"iter_us": us per PCG iteration, "us": {kernel class: us per launch inside the replayed graph}}."""
+    from paper_2508_16298_b200 import hqmc
+    x = g.new_vec()
+    iters = max(64, (iters // 32) * 32)
+
+    def run():
+        g.cg_solve(d_phi, 0.0, iters, x=x)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); g.cg_solve(d_phi, 0.0, iters, x=x); e1.record()
+        torch.cuda.synchronize()
+        return 1e3 * e0.elapsed_time(e1) / iters
+
+    g.set_debug_skip(0)
+    full = run()
+    g.reset_stats(); g.cg_solve(d_phi, 0.0, 32, x=x); torch.cuda.synchronize()
+    used = [k for k in ("mdagm", "cg_axpy", "precond", "cg_dupdate") if g.kernel_stats()[k][0] >= 32]
+    keeper = "cg_dupdate" if "cg_axpy" not in used else "precond"     # the class that counts iterations / sets `done`
+    out = {}
+    for k in used:
+        if k == keeper:
+            continue
+        g.set_debug_skip(1 << hqmc.KERNEL_CLASSES.index(k))
+        out[k] = full - run()
+    g.set_debug_skip(0)
+    out[keeper] = full - sum(out.values())
+    return {"iter_us": full, "us": out}
 
 
 def mdagm_sweep(g, torch, dev, L, Ntau, prec, nbuf=8, reps=25):
@@ -351,7 +371,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number (1-5); 4 = L=48, Ntau=480")
     ap.add_argument("--cg-iters", type=int, default=500, help="fixed PCG iterations per solve (PAPER.md:348)")
-    ap.add_argument("--ref-cg-iters", type=int, default=2, help="PCG iterations per solve of the CPU-oracle sample")
+    ap.add_argument("--ref-cg-iters", type=int, default=60, help="PCG iterations per solve of the CPU-oracle sample")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--prec", default="c128", choices=["c128", "c64"])
     ap.add_argument("--no-sweep", action="store_true")

@@ -141,8 +141,8 @@ int hqmc_set_mdagm_kernel(hqmc_ctx *ctx, int which);
 /* Preconditioner kernel for W = 1..6: n > 0: TMA-tiled kernel, runs of n slices per CTA; n < 0: register-ring
  * kernel with runs of -n slices; 0 = library default (TMA-tiled). */
 int hqmc_set_precond_tile(hqmc_ctx *ctx, int slices_per_run);
-/* PCG vector kernels: 1 (default) = fused residual-update + preconditioner and fused x/d update where the
- * TMA-tiled preconditioner applies (3 kernels per iteration); 0 = the four separate kernels. */
+/* PCG vector kernels: 1 = fused residual-update + preconditioner and fused x/d update where the
+ * TMA-tiled preconditioner applies (3 kernels per iteration); 0 (default) = the four separate kernels. */
 int hqmc_set_cg_fusion(hqmc_ctx *ctx, int on);
 /* TIMING ONLY: bit k of mask set = kernels of class HQMC_K_<k> are not launched (leave-one-out timing of a kernel
  * inside the graph-replayed PCG iteration; the numerical results are then meaningless).  0 restores normal operation. */

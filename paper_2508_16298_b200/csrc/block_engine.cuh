@@ -200,4 +200,24 @@ __device__ __forceinline__ double sum_partials_warp0(const double *__restrict__ 
     return (threadIdx.x < 32) ? sum_partials_lanes(part, n, threadIdx.x) : 0.0;
 }
 
+// Sum n partials with the WHOLE CTA (thread tid of nthreads takes elements tid, tid + nthreads, ... in order, then a
+// fixed shuffle/shared-memory tree): one L2 round trip instead of one per 32 elements.  Every thread gets the result.
+// red: >= 33 doubles of shared memory.  Contains __syncthreads: call from all threads of the CTA.
+__device__ __forceinline__ double cta_sum_partials(const double *__restrict__ part, int n, int tid, int nthreads, double *red) {
+    double s = 0.0;
+    for (int i = tid; i < n; i += nthreads) s += __ldcg(part + i);
+    const int lane = tid & 31, w = tid >> 5, nw = (nthreads + 31) >> 5;
+    s = warp_sum(s);
+    __syncthreads();
+    if (lane == 0) red[w] = s;
+    __syncthreads();
+    if (w == 0) {
+        double r = (lane < nw) ? red[lane] : 0.0;
+        r = warp_sum(r);
+        if (lane == 0) red[32] = r;
+    }
+    __syncthreads();
+    return red[32];
+}
+
 }  // namespace hqmc

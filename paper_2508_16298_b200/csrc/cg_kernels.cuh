@@ -36,13 +36,10 @@ __global__ void k_cg_axpy(size_t N, typename Cx<T>::type *__restrict__ x, typena
                           double *__restrict__ part_rr, const CgState *__restrict__ st) {
     typedef typename Cx<T>::type T2;
     if (*(volatile const int *)&st->done) return;
-    __shared__ double red[32];
-    __shared__ double s_alpha;
-    double rz = sum_partials_warp0(part_rz, n_rz);
-    double dOd = sum_partials_warp0(part_dOd, n_dOd);
-    if (threadIdx.x == 0) s_alpha = rz / dOd;
-    __syncthreads();
-    const T alpha = (T)s_alpha;
+    __shared__ double red[34];
+    const double rz = cta_sum_partials(part_rz, n_rz, threadIdx.x, blockDim.x, red);
+    const double dOd = cta_sum_partials(part_dOd, n_dOd, threadIdx.x, blockDim.x, red);
+    const T alpha = (T)(rz / dOd);
     double acc = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
         T2 xi = x[i], ri = r[i], di = d[i], oi = Od[i];
@@ -188,16 +185,14 @@ __global__ void k_cg_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, con
                              int first, const CgState *__restrict__ st) {
     typedef typename Cx<T>::type T2;
     if (*(volatile const int *)&st->done) return;
-    __shared__ double s_beta;
-    if (first) {
-        if (threadIdx.x == 0) s_beta = 0.0;
-    } else {
-        double a = sum_partials_warp0(part_new, n);
-        double b = sum_partials_warp0(part_old, n);
-        if (threadIdx.x == 0) s_beta = a / b;
+    __shared__ double red[34];
+    double bt = 0.0;
+    if (!first) {
+        const double a = cta_sum_partials(part_new, n, threadIdx.x, blockDim.x, red);
+        const double b = cta_sum_partials(part_old, n, threadIdx.x, blockDim.x, red);
+        bt = a / b;
     }
-    __syncthreads();
-    const T beta = (T)s_beta;
+    const T beta = (T)bt;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
         T2 zi = z[i];
         if (!first) { T2 di = d[i]; zi.x = fma(beta, di.x, zi.x); zi.y = fma(beta, di.y, zi.y); }

@@ -65,7 +65,8 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     c->own_stream = (cuda_stream == nullptr);
     c->stream = (cudaStream_t)cuda_stream;
     c->cg_graph = nullptr; c->cg_graph_x = nullptr; c->cg_graph_tile = 0; c->cg_graph_fused = false; c->cg_chunk = 32;
-    c->profiling = false; c->capturing = false; c->theta_set = false; c->fused_allowed = true; c->cg_fused = false; c->skip_mask = 0;
+    c->profiling = false; c->capturing = false; c->theta_set = false; c->skip_mask = 0; c->cg_fused = false;
+    c->fused_allowed = false;   // fused PCG vector kernels measured no faster at L=48: opt-in
     for (int i = 0; i < HQMC_K_COUNT; ++i) { c->launches[i] = 0; c->graph_nodes[i] = 0; c->ms[i] = 0.0; }
     int st = HQMC_OK;
     auto fail = [&](int s) { hqmc_destroy(c); return s; };

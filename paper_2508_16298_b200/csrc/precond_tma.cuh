@@ -140,8 +140,7 @@ __global__ void __launch_bounds__(SITES * 6, 3) k_cg_rz(Geo g, Taps taps, const 
     static_assert(W >= 1 && W <= 6, "4 + 2W <= 16 tile rows per thread");
     if (*(volatile const int *)&st->done) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ double red[32];
-    __shared__ double s_alpha;
+    __shared__ double red[34];
     __shared__ __align__(8) uint64_t bars[HQMC_PC_MAX_BARS];
     const int Vs = g.Vs, Nt = g.Nt;
     const int tid = threadIdx.y * SITES + threadIdx.x, nthreads = SITES * blockDim.y;
@@ -170,12 +169,10 @@ __global__ void __launch_bounds__(SITES * 6, 3) k_cg_rz(Geo g, Taps taps, const 
         bulk_g2s(tile_r + (size_t)tid * SITES, r_in + (size_t)u * Vs + s0, row_bytes, bar);
         bulk_g2s(tile_o + (size_t)tid * SITES, Od + (size_t)u * Vs + s0, row_bytes, bar);
     }
-    if (tid < 32) {   // alpha, identical in every CTA (fixed-order sums of the producers' partials)
-        const double rz = sum_partials_lanes(part_rz_old, n_rz, tid), dOd = sum_partials_lanes(part_dOd, n_dOd, tid);
-        if (tid == 0) s_alpha = rz / dOd;
-    }
-    __syncthreads();
-    const T alpha = (T)s_alpha;
+    // alpha, identical in every CTA (fixed-order sums of the producers' partials, all threads loading at once)
+    const double rz_old = cta_sum_partials(part_rz_old, n_rz, tid, nthreads, red);
+    const double dOd_tot = cta_sum_partials(part_dOd, n_dOd, tid, nthreads, red);
+    const T alpha = (T)(rz_old / dOd_tot);
     const int i0 = 4 * threadIdx.y;                                      // first tile row / first output (relative to ta)
     double zx[4] = {0, 0, 0, 0}, zy[4] = {0, 0, 0, 0};
     T2 cen[4];
@@ -233,15 +230,11 @@ __global__ void __launch_bounds__(256) k_cg_xd(size_t N, typename Cx<T>::type *_
                         const double *__restrict__ part_rr, CgState *st) {
     typedef typename Cx<T>::type T2;
     if (*(volatile const int *)&st->done) return;
-    __shared__ double s_ab[2];
-    {
-        const double rz_old = sum_partials_warp0(part_rz_old, n_rz);
-        const double rz_new = sum_partials_warp0(part_rz_new, n_rz);
-        const double dOd = sum_partials_warp0(part_dOd, n_dOd);
-        if (threadIdx.x == 0) { s_ab[0] = rz_old / dOd; s_ab[1] = rz_new / rz_old; }
-    }
-    __syncthreads();
-    const T alpha = (T)s_ab[0], beta = (T)s_ab[1];
+    __shared__ double red[34];
+    const double rz_old = cta_sum_partials(part_rz_old, n_rz, threadIdx.x, blockDim.x, red);
+    const double rz_new = cta_sum_partials(part_rz_new, n_rz, threadIdx.x, blockDim.x, red);
+    const double dOd = cta_sum_partials(part_dOd, n_dOd, threadIdx.x, blockDim.x, red);
+    const T alpha = (T)(rz_old / dOd), beta = (T)(rz_new / rz_old);
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     for (; i + stride < N; i += 2 * stride) {          // two independent elements in flight per thread
@@ -257,7 +250,7 @@ __global__ void __launch_bounds__(256) k_cg_xd(size_t N, typename Cx<T>::type *_
         x[i] = x0; d[i] = d0;
     }
     if (blockIdx.x == 0) {
-        const double rr = sum_partials_warp0(part_rr, n_rz);
+        const double rr = cta_sum_partials(part_rr, n_rz, threadIdx.x, blockDim.x, red);
         if (threadIdx.x == 0) {
             const long long it = st->iters + 1;
             st->iters = it; st->rr = rr;
