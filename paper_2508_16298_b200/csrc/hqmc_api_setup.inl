@@ -109,12 +109,13 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     }
     if (c->use_stream) {
         ALLOC(c->d_packed, 2 * c->N * 8);
-        ALLOC(c->d_tab, sizeof(double2) * 2 * HQMC_PHASE_K);
-        std::vector<double2> tab((size_t)2 * HQMC_PHASE_K);
+        ALLOC(c->d_tab, sizeof(double2) * 2 * HQMC_PHASE_TAB);
+        std::vector<double2> tab((size_t)2 * HQMC_PHASE_TAB);
         for (int s2 = 0; s2 < 2; ++s2)
             for (int k = 0; k < HQMC_PHASE_K; ++k) {
                 const double ang = 2.0 * M_PI * (double)k / (double)HQMC_PHASE_K, sc = s2 ? c->th_full : c->th_half;
-                tab[(size_t)s2 * HQMC_PHASE_K + k] = make_double2(sc * std::cos(ang), sc * std::sin(ang));
+                for (int rep = 0; rep < HQMC_PHASE_REP; ++rep)    // 8 replicas: bank-conflict-free lookups (mdagm_stream.cuh)
+                    tab[(size_t)s2 * HQMC_PHASE_TAB + (size_t)k * HQMC_PHASE_REP + rep] = make_double2(sc * std::cos(ang), sc * std::sin(ang));
             }
         cudaError_t e = cudaMemcpy(c->d_tab, tab.data(), sizeof(double2) * tab.size(), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) { g_last_error = cudaGetErrorString(e); return fail(HQMC_ECUDA); }

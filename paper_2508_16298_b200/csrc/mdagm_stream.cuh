@@ -21,37 +21,43 @@ namespace hqmc {
 
 // ------------------------------------------------------------------------------------------------
 // PhasePack: 8 bytes per link.
-// double:  theta = k*delta + r, delta = 2 pi / 1024, |r| <= delta/2.  The word holds sin(r) as an fp64 with its
-//          10 low mantissa bits replaced by k (sin r < 2^-8, so the absolute error of the stored sine is
-//          <= 2^-8 * 2^-43 = 4.4e-16 ... 1.1e-16 after rounding to nearest -- one ulp of a unit phase).
-//          Decode: cos r = 1 - q/2 - q^2/8 (q = sin^2 r <= 9.5e-6, next term 5e-17), then one complex
-//          multiply with the table entry  tanh(a) e^{i k delta}  (shared memory, 1024 entries per scale a).
+// double:  theta = k*delta + r, delta = 2 pi / 128, |r| <= delta/2.  The word holds sin(r) as an fp64 with its
+//          7 low mantissa bits replaced by k (sin r < 2^-5, so the absolute error of the stored sine is
+//          <= 2^-5 * 2^-47 = 2.2e-16 before rounding to nearest, 1.1e-16 after -- half an ulp of a unit phase).
+//          Decode: cos r = sqrt(1 - q) = 1 - q/2 - q^2/8 - q^3/16 - 5 q^4/128 (q = sin^2 r <= 6.1e-4, next term
+//          2e-18), then one complex multiply with the table entry  tanh(a) e^{i k delta}.  The table lives in shared
+//          memory with every entry replicated 8 times (128 entries x 8 x 16 B per scale a): lane l reads replica
+//          l & 7, so the 8 lanes of a quarter warp always hit 8 different 16-byte bank groups -- the random lookups
+//          are bank-conflict free.
 // float:   the scaled phase itself as float2 (8 bytes), no decoding.
 // ------------------------------------------------------------------------------------------------
-#define HQMC_PHASE_K 1024
+#define HQMC_PHASE_K 128
+#define HQMC_PHASE_REP 8
+#define HQMC_PHASE_TAB (HQMC_PHASE_K * HQMC_PHASE_REP)      // double2 elements per scale
 
 template <typename T> struct PhasePack;
 template <> struct PhasePack<double> {
     typedef unsigned long long word;
     static __device__ __forceinline__ word pack(double theta, double /*scale*/) {
-        const double inv_delta = 162.97466172610083;       // 1024 / (2 pi)
-        const double d_hi = 0.006135923151542565;           // fp64(2 pi / 1024)
-        const double d_lo = 2.391888279584674e-19;           // 2 pi / 1024 - d_hi
+        const double inv_delta = 20.371832715762603;         // 128 / (2 pi)
+        const double d_hi = 0.04908738521234052;             // fp64(2 pi / 128)
+        const double d_lo = 1.9135106236677392e-18;          // 2 pi / 128 - d_hi
         double kf = rint(theta * inv_delta);
         double r = fma(-kf, d_hi, theta);
         r = fma(-kf, d_lo, r);
         long long k = (long long)kf;
         double s = sin(r);
         unsigned long long u = (unsigned long long)__double_as_longlong(s);
-        u = (u + 512ull) & ~1023ull;                         // round the mantissa to 43 bits
-        return u | (unsigned long long)(k & 1023ll);
+        u = (u + 64ull) & ~127ull;                           // round the mantissa to 46 bits
+        return u | (unsigned long long)(k & 127ll);
     }
+    // tab: this scale's table, already offset by the calling lane's replica (lane & 7)
     static __device__ __forceinline__ double2 decode(word u, const double2 *__restrict__ tab) {
-        const unsigned k = (unsigned)u & 1023u;
-        const double sr = __longlong_as_double((long long)(u & ~1023ull));
+        const unsigned k = (unsigned)u & 127u;
+        const double sr = __longlong_as_double((long long)(u & ~127ull));
         const double q = sr * sr;
-        const double cr = fma(q, fma(q, -0.125, -0.5), 1.0);
-        const double2 t = tab[k];
+        const double cr = fma(q, fma(q, fma(q, fma(q, -0.0390625, -0.0625), -0.125), -0.5), 1.0);
+        const double2 t = tab[k * HQMC_PHASE_REP];
         double2 P;
         P.x = fma(-t.y, sr, t.x * cr);
         P.y = fma(t.x, sr, t.y * cr);
@@ -177,10 +183,28 @@ template <typename T>
 __device__ __forceinline__ void lean_load_phases(const unsigned char *pbuf, const double2 *tab, int nb, int q, LeanPh<typename Cx<T>::type> &P) {
     const unsigned char *p = pbuf + (size_t)q * 16;
     const size_t st = (size_t)nb * 16;
+    tab += threadIdx.x & (HQMC_PHASE_REP - 1);             // this lane's replica of the table
     PackLoad<T>::pair(p, tab, P.a4, P.b4);
     PackLoad<T>::pair(p + st, tab, P.a3, P.b3);
     PackLoad<T>::pair(p + 2 * st, tab, P.a2, P.b2);
-    PackLoad<T>::pair(p + 3 * st, tab + HQMC_PHASE_K, P.a1, P.b1);
+    PackLoad<T>::pair(p + 3 * st, tab + HQMC_PHASE_TAB, P.a1, P.b1);
+}
+
+// Conflict-free block load / store of the staged slices: a thread's sites (xa, y) and (xb, y) are 16 B apart with a
+// 32 B stride between lanes, so a plain 128-bit access per site is a 2-way bank conflict.  Lanes 4..7 of every
+// quarter warp take the two sites in the opposite order: the 8 lanes then touch 8 different 16-byte bank groups.
+template <typename T2>
+__device__ __forceinline__ void load_block_swz(const T2 *__restrict__ buf, const LeanIdx &b, T2 &v0, T2 &v1, T2 &v2, T2 &v3) {
+    const bool sw = threadIdx.x & 4;
+    const T2 a = buf[sw ? b.o1 : b.o0], c = buf[sw ? b.o0 : b.o1];
+    const T2 d = buf[sw ? b.o3 : b.o2], e = buf[sw ? b.o2 : b.o3];
+    v0 = sw ? c : a; v1 = sw ? a : c; v2 = sw ? e : d; v3 = sw ? d : e;
+}
+template <typename T2>
+__device__ __forceinline__ void store_block_swz(T2 *__restrict__ buf, const LeanIdx &b, const T2 &v0, const T2 &v1, const T2 &v2, const T2 &v3) {
+    const bool sw = threadIdx.x & 4;
+    buf[sw ? b.o1 : b.o0] = sw ? v1 : v0; buf[sw ? b.o0 : b.o1] = sw ? v0 : v1;
+    buf[sw ? b.o3 : b.o2] = sw ? v3 : v2; buf[sw ? b.o2 : b.o3] = sw ? v2 : v3;
 }
 
 template <typename T> struct StreamSmem {
@@ -189,7 +213,7 @@ template <typename T> struct StreamSmem {
     __host__ __device__ StreamSmem(int Vs, int nbp) {
         typedef typename Cx<T>::type T2;
         size_t o = 0;
-        tab = o;  o += (sizeof(T) == 8) ? (size_t)2 * HQMC_PHASE_K * sizeof(double2) : 0;
+        tab = o;  o += (sizeof(T) == 8) ? (size_t)2 * HQMC_PHASE_TAB * sizeof(double2) : 0;
         vbuf = o; o += (size_t)Vs * sizeof(T2);
         vbuf2 = o; o += (size_t)Vs * sizeof(T2);
         pbuf = o; o += (size_t)2 * Vs * 8;
@@ -248,7 +272,7 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
     if (leader) {
         mbar_init(bar_v, 1); mbar_init(bar_v2, 1); mbar_init(bar_p, 1); mbar_init(bar_t, 1);
         mbar_fence_init();
-        if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_K * sizeof(double2), bar_t);
+        if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_TAB * sizeof(double2), bar_t);
         bulk_load(smem_raw + lay.vbuf, in_b + (size_t)tp * vbytes, vbytes, bar_v);
         bulk_load(pbuf, pk_b + (size_t)tp * pbytes, pbytes, bar_p);
         bulk_load(smem_raw + lay.vbuf2, in_b + (size_t)t0 * vbytes, vbytes, bar_v2);
@@ -269,7 +293,7 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
     // ---- prologue: w_{t0} = v_{t0} - sigma_{tp} C B_{tp} v_{tp}
     mbar_wait(bar_v, par_vA); par_vA ^= 1;
     mbar_wait(bar_p, par_p); par_p ^= 1;
-    w0 = vsA[b.o0]; w1 = vsA[b.o1]; w2 = vsA[b.o2]; w3 = vsA[b.o3];
+    load_block_swz(vsA, b, w0, w1, w2, w3);
     lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
     lean_apply_B(ex, nbp, b, P, w0, w1, w2, w3, [&]() {
         if (leader) {                     // buffer A and pbuf have been read by everyone
@@ -281,7 +305,8 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
         const T sC = (tp == g.Nt - 1) ? C : -C;
         mbar_wait(bar_v2, par_vB); par_vB ^= 1;
         mbar_wait(bar_p, par_p); par_p ^= 1;
-        T2 v0 = vsB[b.o0], v1 = vsB[b.o1], v2 = vsB[b.o2], v3 = vsB[b.o3];
+        T2 v0, v1, v2, v3;
+        load_block_swz(vsB, b, v0, v1, v2, v3);
         w0.x = fma(sC, w0.x, v0.x); w0.y = fma(sC, w0.y, v0.y); w1.x = fma(sC, w1.x, v1.x); w1.y = fma(sC, w1.y, v1.y);
         w2.x = fma(sC, w2.x, v2.x); w2.y = fma(sC, w2.y, v2.y); w3.x = fma(sC, w3.x, v3.x); w3.y = fma(sC, w3.y, v3.y);
         lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
@@ -297,7 +322,8 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
         // v = B_t v_t / C.  After the first barrier of the sweep sequence everyone has read v_t and (at the end of the
         // previous iteration) the links, and obuf holds out_{t-1} completely: thread 0 stores it and fetches v_{t+2}
         // into the buffer v_t occupied and the links of slice t+1.
-        T2 v0 = vcur[b.o0], v1 = vcur[b.o1], v2 = vcur[b.o2], v3 = vcur[b.o3];
+        T2 v0, v1, v2, v3;
+        load_block_swz(vcur, b, v0, v1, v2, v3);
         lean_apply_B(ex, nbp, b, P, v0, v1, v2, v3, [&]() {
             if (leader) {
                 if (i > 0) { bulk_s2g(out_b + (size_t)(t - 1) * vbytes, osm, vbytes); bulk_commit(); }
@@ -308,7 +334,8 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
             }
         });
         if (odd) { mbar_wait(bar_v2, par_vB); par_vB ^= 1; } else { mbar_wait(bar_v, par_vA); par_vA ^= 1; }
-        T2 n0 = vnxt[b.o0], n1 = vnxt[b.o1], n2 = vnxt[b.o2], n3 = vnxt[b.o3];   // v_{t+1}
+        T2 n0, n1, n2, n3;                                                         // v_{t+1}
+        load_block_swz(vnxt, b, n0, n1, n2, n3);
         T2 q0, q1, q2, q3;                                                         // w_{t+1}, then B_t w_{t+1}
         q0.x = fma(sC, v0.x, n0.x); q0.y = fma(sC, v0.y, n0.y); q1.x = fma(sC, v1.x, n1.x); q1.y = fma(sC, v1.y, n1.y);
         q2.x = fma(sC, v2.x, n2.x); q2.y = fma(sC, v2.y, n2.y); q3.x = fma(sC, v3.x, n3.x); q3.y = fma(sC, v3.y, n3.y);
@@ -323,7 +350,7 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename P
         q0.x = fma(sC, q0.x, w0.x); q0.y = fma(sC, q0.y, w0.y); q1.x = fma(sC, q1.x, w1.x); q1.y = fma(sC, q1.y, w1.y);
         q2.x = fma(sC, q2.x, w2.x); q2.y = fma(sC, q2.y, w2.y); q3.x = fma(sC, q3.x, w3.x); q3.y = fma(sC, q3.y, w3.y);
         w0 = k0; w1 = k1; w2 = k2; w3 = k3;
-        if (b.act) { osm[b.o0] = q0; osm[b.o1] = q1; osm[b.o2] = q2; osm[b.o3] = q3; }
+        if (b.act) store_block_swz(osm, b, q0, q1, q2, q3);
         fence_async_smem();               // my obuf writes -> visible to the async proxy (the store is issued after the next barrier)
         if (more) {
             mbar_wait(bar_p, par_p); par_p ^= 1;

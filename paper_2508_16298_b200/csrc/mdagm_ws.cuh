@@ -41,7 +41,7 @@ template <typename T> struct WsSmem {
     __host__ __device__ WsSmem(int Vs, int nbp, int h, int ns) {
         typedef typename Cx<T>::type T2;
         size_t o = 0;
-        tab = o;  o += (sizeof(T) == 8) ? (size_t)2 * HQMC_PHASE_K * sizeof(double2) : 0;
+        tab = o;  o += (sizeof(T) == 8) ? (size_t)2 * HQMC_PHASE_TAB * sizeof(double2) : 0;
         vbuf[0] = o; o += (size_t)Vs * sizeof(T2);
         vbuf[1] = o; o += (size_t)Vs * sizeof(T2);
         pbuf = o; o += (size_t)2 * Vs * 8;
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(608, 1) k_mdagm_ws(Geo g, const typename Phase
         mbar_init(emp_v, ncw); mbar_init(emp_v + 1, ncw); mbar_init(emp_p, ncw); mbar_init(full_o, ncw); mbar_init(emp_o, 1);
         for (int i = 0; i < 2 * wg.ns; ++i) mbar_init(ebar + i, g.h);
         mbar_fence_init();
-        if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_K * sizeof(double2), bar_t);
+        if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_TAB * sizeof(double2), bar_t);
         bulk_load(smem_raw + lay.vbuf[0], in_b + (size_t)tp * vbytes, vbytes, full_v);
         bulk_load(pbuf, pk_b + (size_t)tp * pbytes, pbytes, full_p);
         bulk_load(smem_raw + lay.vbuf[1], in_b + (size_t)t0 * vbytes, vbytes, full_v + 1);
