@@ -336,6 +336,33 @@ def pcg_kernel_costs(g, torch, d_phi, iters):
     return {"iter_us": full, "us": out}
 
 
+def run_solve(args):
+    """--mode solve: one preconditioned CG solve to --tol on the chosen config (BASELINE.json: "CG-solve ms ... iteration
+    count and ms per solve reported"), plus the same solve without the preconditioner capped at the same iteration count."""
+    import torch
+    from paper_2508_16298_b200 import hqmc, inputs
+    c = inputs.CONFIGS[args.config]
+    L, Ntau = c["L"], c["Ntau"]
+    theta = inputs.make_theta(args.config)
+    eta = inputs.complex_gaussian((Ntau, L, L), c["seed"])
+    out = {"mode": "solve", "config": args.config, "L": L, "Ntau": Ntau, "tol": args.tol, "theta": c["theta"]}
+    for W in (6, 0):
+        g = hqmc.HQMC(L, Ntau, W=W)
+        g.set_theta(torch.from_numpy(theta).cuda())
+        phi = g.apply_Mdag(torch.from_numpy(eta).cuda())
+        cap = args.max_iter if W else out["W6"]["iters"]
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        x, it, rel, ok = g.cg_solve(phi, args.tol, cap)
+        torch.cuda.synchronize(); dt = time.perf_counter() - t0
+        true_res = float(torch.linalg.vector_norm(phi - g.apply_MdagM(x)) / torch.linalg.vector_norm(phi))
+        out[f"W{W}"] = {"iters": it, "converged": ok, "recurrence_relres": rel, "true_relres": true_res, "ms_per_solve": 1e3 * dt,
+                        "us_per_iter": 1e6 * dt / max(1, it), "SF_minus_eta2": float((torch.vdot(phi.ravel(), x.ravel()).real
+                                                                                     - (abs(torch.from_numpy(eta)) ** 2).sum()))}
+        g.close()
+    print(json.dumps(out))
+    return 0
+
+
 def mdagm_sweep(g, torch, dev, L, Ntau, prec, nbuf=8, reps=25):
     """M^+M alone: cold = rotate nbuf distinct (in, out) pairs so every launch streams from HBM; warm = one pair."""
     N = L * L * Ntau
@@ -375,9 +402,14 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--prec", default="c128", choices=["c128", "c64"])
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--mode", default="step", choices=["step", "solve"], help="solve: one full PCG solve to --tol (not the timed metric)")
+    ap.add_argument("--tol", type=float, default=1e-10)
+    ap.add_argument("--max-iter", type=int, default=3000000)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3
+    if args.mode == "solve":
+        return run_solve(args)
     return run_reference(args) if args.impl == "reference" else run_gpu(args)
 
 

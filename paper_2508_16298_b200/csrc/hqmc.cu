@@ -102,7 +102,7 @@ template <typename T> static int do_phase(hqmc_ctx *c, const double *p, double t
                          (T2 *)c->d_ph, c->th_full, c->th_half));
     else HQ_TRY(launch(c, HQMC_K_PHASE, k_phase<T, false>, dim3(c->grid_ew), dim3(256), 0, c->g, c->d_theta, (const double *)nullptr,
                        0.0, (T2 *)c->d_ph, c->th_full, c->th_half));
-    if (c->use_stream)
+    if (c->use_stream || c->use_cluster)
         HQ_TRY(launch(c, HQMC_K_PHASE, k_phase_pack<T>, dim3(c->grid_ew), dim3(256), 0, c->g, (const double *)c->d_theta,
                       (W *)c->d_packed, c->th_full, c->th_half));
     return HQMC_OK;
@@ -136,8 +136,55 @@ template <typename T> static int do_mdagm_stream(hqmc_ctx *c, const void *in, vo
                   (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st);
 }
 
+// cluster launch (cudaLaunchKernelEx with a cluster dimension); same bookkeeping as launch()
+template <typename... KArgs, typename... Args>
+static int launch_cluster(hqmc_ctx *c, int kclass, void (*kernel)(KArgs...), int grid, int block, size_t smem, int R, Args... args) {
+    if (c->skip_mask & (1u << kclass)) return HQMC_OK;
+    if (c->capturing) c->graph_nodes[kclass]++; else c->launches[kclass]++;
+    const bool prof = c->profiling && !c->capturing;
+    EventPair ep{};
+    if (prof) {
+        if (c->pending.size() >= 2048) HQ_TRY(drain_events(c));
+        if (!c->pool.empty()) { ep = c->pool.back(); c->pool.pop_back(); }
+        else { CUDA_TRY(cudaEventCreate(&ep.a)); CUDA_TRY(cudaEventCreate(&ep.b)); }
+        ep.kclass = kclass;
+        CUDA_TRY(cudaEventRecord(ep.a, c->stream));
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = R; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...));
+    if (prof) { CUDA_TRY(cudaEventRecord(ep.b, c->stream)); c->pending.push_back(ep); }
+    return HQMC_OK;
+}
+
+template <typename T> static int do_mdagm_cluster(hqmc_ctx *c, const void *in, void *out, bool dot, const CgState *st) {
+    typedef typename Cx<T>::type T2;
+    typedef typename PhasePack<T>::word W;
+    const int R = c->cl_R;
+    int Gc = c->time_tile > 0 ? (c->g.Nt + c->time_tile - 1) / c->time_tile : (c->g.Nt < c->n_sm / R ? c->g.Nt : c->n_sm / R);
+    if (Gc < 1) Gc = 1;
+    c->grid_mdagm = Gc * R;
+    auto go = [&](auto kern_dot, auto kern_plain) -> int {
+        if (dot) {
+            CUDA_TRY(cudaFuncSetAttribute(kern_dot, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->cl_smem));
+            return launch_cluster(c, HQMC_K_MDAGM, kern_dot, Gc * R, c->cl_threads, c->cl_smem, R, c->g, (const W *)c->d_packed,
+                                  (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, c->d_part_dOd, st);
+        }
+        CUDA_TRY(cudaFuncSetAttribute(kern_plain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->cl_smem));
+        return launch_cluster(c, HQMC_K_MDAGM, kern_plain, Gc * R, c->cl_threads, c->cl_smem, R, c->g, (const W *)c->d_packed,
+                              (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st);
+    };
+    if (c->cl_threads <= 512) return go(k_mdagm_cluster<T, true, 512>, k_mdagm_cluster<T, false, 512>);   // 128 registers per thread
+    return go(k_mdagm_cluster<T, true, 576>, k_mdagm_cluster<T, false, 576>);
+}
+
 template <typename T> static int do_mdagm(hqmc_ctx *c, const void *in, void *out, bool dot, const CgState *st) {
     typedef typename Cx<T>::type T2;
+    if (c->use_cluster && c->cluster_on) return do_mdagm_cluster<T>(c, in, out, dot, st);
     if (c->use_stream && c->stream_on) return do_mdagm_stream<T>(c, in, out, dot, st);
     const int Tt = c->time_tile;
     const int grid = (c->g.Nt + Tt - 1) / Tt;

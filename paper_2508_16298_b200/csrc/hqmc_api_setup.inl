@@ -106,8 +106,19 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
                                               : WsSmem<float>(c->g.Vs, c->cfg.threads, h, ws_ns).total;
         c->use_ws = c->use_stream && c->cfg.threads + 32 <= 608 && c->ws_smem <= (size_t)prop.sharedMemPerBlockOptin;
         c->ws_on = false;   // measured slower than k_mdagm_stream (profiles/): kept selectable
+        // cluster kernel: the slice split over R SMs (smallest R whose strip fits one SM's threads and shared memory)
+        c->use_cluster = false; c->cluster_on = false; c->cl_R = 0;
+        for (int R = 2; R <= 8 && !c->use_cluster; R *= 2) {
+            if (h % R) continue;
+            const int thr = ((h / R) * h + 31) / 32 * 32;
+            const size_t sm = (prm->prec == HQMC_C128) ? ClusterSmem<double>(prm->L, h, R, thr).total : ClusterSmem<float>(prm->L, h, R, thr).total;
+            if (thr <= 576 && sm <= (size_t)prop.sharedMemPerBlockOptin && (size_t)c->g.Vs * 16 < (1u << 20)) {
+                c->use_cluster = true; c->cl_R = R; c->cl_threads = thr; c->cl_smem = sm;
+            }
+        }
+        c->cluster_on = c->use_cluster && !c->use_stream;      // default only where one SM cannot hold the slice
     }
-    if (c->use_stream) {
+    if (c->use_stream || c->use_cluster) {
         ALLOC(c->d_packed, 2 * c->N * 8);
         ALLOC(c->d_tab, sizeof(double2) * 2 * HQMC_PHASE_TAB);
         std::vector<double2> tab((size_t)2 * HQMC_PHASE_TAB);
@@ -134,7 +145,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     if (st != HQMC_OK) return fail(st);
     st = DISPATCH_T(c, auto_time_tile<double>(c), auto_time_tile<float>(c));
     if (st != HQMC_OK) return fail(st);
-    if (c->use_stream) c->time_tile = 0;
+    if (c->use_stream || c->cluster_on) c->time_tile = 0;
     st = build_default_taps(c);
     if (st != HQMC_OK) return fail(st);
     precond_cfg(c, 0);
@@ -230,7 +241,7 @@ extern "C" int hqmc_get_kernel_stats(hqmc_ctx *c, int which, long long *launches
 extern "C" int hqmc_set_time_tile(hqmc_ctx *c, int tt) {
     if (!c || tt < 0 || tt > c->g.Nt) return HQMC_EINVAL;
     if (tt == 0) {
-        if (c->use_stream && c->stream_on) { c->time_tile = 0; return HQMC_OK; }   // one CTA per SM, slices dealt out evenly
+        if ((c->use_stream && c->stream_on) || c->cluster_on) { c->time_tile = 0; return HQMC_OK; }   // one CTA per SM, slices dealt out evenly
         return DISPATCH_T(c, auto_time_tile<double>(c), auto_time_tile<float>(c));
     }
     if ((c->g.Nt + tt - 1) / tt > HQMC_MAX_PART) return HQMC_EINVAL;
@@ -257,10 +268,11 @@ extern "C" int hqmc_set_cg_fusion(hqmc_ctx *c, int on) {
     return HQMC_OK;
 }
 extern "C" int hqmc_set_mdagm_kernel(hqmc_ctx *c, int which) {
-    if (!c || which < 0 || which > 2) return HQMC_EINVAL;
-    if ((which == 0 && !c->use_stream) || (which == 2 && !c->use_ws)) return HQMC_EINVAL;
-    c->stream_on = (which != 1);
+    if (!c || which < 0 || which > 3) return HQMC_EINVAL;
+    if ((which == 0 && !c->use_stream) || (which == 2 && !c->use_ws) || (which == 3 && !c->use_cluster)) return HQMC_EINVAL;
+    c->stream_on = (which == 0 || which == 2);
     c->ws_on = (which == 2);
+    c->cluster_on = (which == 3);
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     return hqmc_set_time_tile(c, 0);
 }

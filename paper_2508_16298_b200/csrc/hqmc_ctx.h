@@ -15,6 +15,7 @@
 #include "kernels.cuh"
 #include "mdagm_stream.cuh"
 #include "mdagm_ws.cuh"
+#include "mdagm_cluster.cuh"
 #include "precond_tma.cuh"
 
 namespace hqmc {
@@ -61,6 +62,8 @@ struct hqmc_ctx {
     double2 *d_tab;      // [2][1024] tanh(a) e^{i k delta} (half step, full step)
     bool stream_on;      // runtime switch (hqmc_set_mdagm_kernel): a streaming kernel is selected
     bool use_ws, ws_on;  // warp-specialised strip kernel usable / selected
+    bool use_cluster, cluster_on;   // cluster kernel (slice split over R SMs) usable / selected
+    int cl_R, cl_threads; size_t cl_smem;
     size_t ws_smem;
     bool use_stream;     // streaming kernel usable (BPT == 1 and its shared memory fits)
     size_t stream_smem;

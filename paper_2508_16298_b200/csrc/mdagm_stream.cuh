@@ -193,15 +193,15 @@ __device__ __forceinline__ void lean_load_phases(const unsigned char *pbuf, cons
 // Conflict-free block load / store of the staged slices: a thread's sites (xa, y) and (xb, y) are 16 B apart with a
 // 32 B stride between lanes, so a plain 128-bit access per site is a 2-way bank conflict.  Lanes 4..7 of every
 // quarter warp take the two sites in the opposite order: the 8 lanes then touch 8 different 16-byte bank groups.
-template <typename T2>
-__device__ __forceinline__ void load_block_swz(const T2 *__restrict__ buf, const LeanIdx &b, T2 &v0, T2 &v1, T2 &v2, T2 &v3) {
+template <typename T2, typename Idx>
+__device__ __forceinline__ void load_block_swz(const T2 *__restrict__ buf, const Idx &b, T2 &v0, T2 &v1, T2 &v2, T2 &v3) {
     const bool sw = threadIdx.x & 4;
     const T2 a = buf[sw ? b.o1 : b.o0], c = buf[sw ? b.o0 : b.o1];
     const T2 d = buf[sw ? b.o3 : b.o2], e = buf[sw ? b.o2 : b.o3];
     v0 = sw ? c : a; v1 = sw ? a : c; v2 = sw ? e : d; v3 = sw ? d : e;
 }
-template <typename T2>
-__device__ __forceinline__ void store_block_swz(T2 *__restrict__ buf, const LeanIdx &b, const T2 &v0, const T2 &v1, const T2 &v2, const T2 &v3) {
+template <typename T2, typename Idx>
+__device__ __forceinline__ void store_block_swz(T2 *__restrict__ buf, const Idx &b, const T2 &v0, const T2 &v1, const T2 &v2, const T2 &v3) {
     const bool sw = threadIdx.x & 4;
     buf[sw ? b.o1 : b.o0] = sw ? v1 : v0; buf[sw ? b.o0 : b.o1] = sw ? v0 : v1;
     buf[sw ? b.o3 : b.o2] = sw ? v3 : v2; buf[sw ? b.o2 : b.o3] = sw ? v2 : v3;

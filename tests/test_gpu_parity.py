@@ -35,7 +35,8 @@ def setup(hq, L, Nt, seed, theta=None, **kw):
 
 
 # sizes: tiny (config 1), odd-shaped, several warps with ragged thread tail, BPT=2 and BPT=4 code paths
-SHAPES = [(4, 8, 0), (6, 10, 1), (12, 14, 2), (18, 7, 3), (34, 5, 4), (50, 4, 5), (70, 3, 6)]
+SHAPES = [(4, 8, 0), (6, 10, 1), (12, 14, 2), (18, 7, 3), (34, 5, 4), (50, 4, 5), (70, 3, 6), (16, 9, 7), (64, 5, 8), (48, 7, 9),
+          (96, 3, 10)]
 
 
 @pytest.mark.parametrize("L,Nt,seed", SHAPES)
@@ -47,11 +48,12 @@ def test_M_Mdag_MdagM(hq, L, Nt, seed):
     assert rel(g.apply_Mdag(dv).cpu().numpy(), o.apply_Mdag(theta, v)) <= 1e-12
     ref = o.apply_MdagM(theta, v)
     assert rel(g.apply_MdagM(dv).cpu().numpy(), ref) <= 1e-12
-    for which in (2, 0, 1):           # 2: warp-specialised strips, 0: streaming (TMA) kernel (both where they fit), 1: register-only
+    for which in (3, 2, 0, 1):        # 3: cluster (DSMEM) kernel, 2: warp-specialised strips, 0: streaming (TMA) kernel, 1: register-only
         try:
             g.set_mdagm_kernel(which)
-        except hq.HqmcError:
-            assert which in (0, 2) and L > 48
+        except hq.HqmcError:      # not available for this lattice: streaming kernels need the slice on one SM (L <= 48),
+            assert which != 1      # the cluster kernel an even number of block-rows and a strip that fits one SM
+            assert (which in (0, 2) and L > 48) or (which == 3 and ((L // 2) % 2 or L > 96))
             continue
         for tt in (0, 1, 2, 3, Nt):   # default split and every time-tile shape incl. ragged last tile and one-CTA-for-all
             g.set_time_tile(tt)
