@@ -208,3 +208,46 @@ def test_host_buffer_entry_points(hq):
     _, it, relres, ok = g.cg_solve_host(theta, v, x, 1e-10, 10000)
     assert ok and rel(x, o.pcg(theta, v, 1e-13, 10000)[0]) <= 1e-9
     g.close()
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_configs_in_bench_launch_configuration(hq, cfg):
+    """BASELINE configs 3-5 at FULL size, default kernels (what bench.py times: streaming kernel at L <= 48, cluster kernel
+    at L = 64): M, M^+, M^+M, P and the force element by element against the oracle, and 20 fixed-count PCG iterations."""
+    c = inputs.CONFIGS[cfg]
+    L, Nt = c["L"], c["Ntau"]
+    theta = inputs.theta_uniform(L, Nt, c["seed"])      # config 5's heat-bath field costs minutes of CPU: uniform stands in here
+    o, g, _ = setup(hq, L, Nt, c["seed"], theta=theta)
+    v = inputs.complex_gaussian((Nt, L, L), c["seed"], inputs.STREAM_VEC)
+    dv = dev(v)
+    assert rel(g.apply_M(dv).cpu().numpy(), o.apply_M(theta, v)) <= 1e-12
+    assert rel(g.apply_Mdag(dv).cpu().numpy(), o.apply_Mdag(theta, v)) <= 1e-12
+    assert rel(g.apply_MdagM(dv).cpu().numpy(), o.apply_MdagM(theta, v)) <= 1e-12
+    assert rel(g.precond(dv).cpu().numpy(), o.precond(v)) <= 1e-13
+    gF = g.force(dv).cpu().numpy()
+    ref = o.force_fermion(theta, v)
+    assert np.abs(gF - ref).max() <= 1e-9 * max(1.0, np.abs(ref).max())
+    xf, itf, relf, _ = g.cg_solve(dv, 0.0, 20)
+    xo, ito, relo = o.pcg(theta, v, 0.0, 20)
+    assert itf == ito == 20 and rel(xf.cpu().numpy(), xo) <= 1e-10 and abs(relf - relo) <= 1e-9 * relo
+    g.close()
+
+
+def test_config3_full_size_trajectory_fixed_count(hq):
+    """BASELINE config 3 (L=24, Ntau=240, uniform theta, eps=0.05) at full size: leapfrog steps with the paper's fixed-count
+    CG protocol (40 iterations per solve on both sides, so both run the same arithmetic path -- converging
+    this field to 1e-13 takes ~1e5 iterations per solve, hours for the oracle): theta', p' and H agree."""
+    c = inputs.CONFIGS[3]
+    L, Nt, nsteps = c["L"], c["Ntau"], 3
+    o, g, theta = setup(hq, L, Nt, c["seed"])
+    eta = inputs.complex_gaussian((Nt, L, L), c["seed"])
+    phi = o.apply_Mdag(theta, eta)
+    p = inputs.momenta(L, Nt, c["seed"])
+    ref = o.trajectory(theta, p, phi, nsteps, 0.05, cg_tol=0.0, cg_max_iter=40)
+    dth, dp = dev(theta), dev(p)
+    r = g.trajectory(dth, dp, dev(phi), nsteps, 0.05, cg_tol=0.0, cg_max_iter=40)
+    assert r["cg_iters"] == ref["cg_iters"] == 40 * (nsteps + 1)
+    assert np.abs(dth.cpu().numpy() - ref["theta"]).max() <= 1e-10
+    assert np.abs(dp.cpu().numpy() - ref["p"]).max() <= 1e-9 * max(1.0, np.abs(ref["p"]).max())
+    assert abs(r["H0"] - ref["H0"]) <= 1e-10 * abs(ref["H0"]) and abs(r["H1"] - ref["H1"]) <= 1e-10 * abs(ref["H1"])
+    g.close()
