@@ -251,3 +251,34 @@ def test_config3_full_size_trajectory_fixed_count(hq):
     assert np.abs(dp.cpu().numpy() - ref["p"]).max() <= 1e-9 * max(1.0, np.abs(ref["p"]).max())
     assert abs(r["H0"] - ref["H0"]) <= 1e-10 * abs(ref["H0"]) and abs(r["H1"] - ref["H1"]) <= 1e-10 * abs(ref["H1"])
     g.close()
+
+
+@pytest.mark.parametrize("L,Nt", [(48, 37), (64, 21), (12, 30)])
+def test_kernels_are_deterministic_run_to_run(hq, L, Nt):
+    """Race / ordering detector for the TMA + mbarrier pipelines (compute-sanitizer is closed on this pool): every M^+M
+    kernel variant gives BITWISE the same vector on 40 back-to-back launches, and a fixed-count PCG solve (fixed-order
+    reductions, no atomics) gives bitwise the same iterate twice."""
+    theta = inputs.theta_uniform(L, Nt, 11)
+    g = hq.HQMC(L, Nt)
+    g.set_theta(dev(theta))
+    v = dev(inputs.complex_gaussian((Nt, L, L), 11, inputs.STREAM_VEC))
+    for which in (0, 2, 3, 1):
+        try:
+            g.set_mdagm_kernel(which)
+        except hq.HqmcError:
+            continue
+        ref = g.apply_MdagM(v).clone()
+        out = g.new_vec()
+        for rep in range(40):
+            g.apply_MdagM(v, out)
+            assert torch.equal(out, ref), (which, rep)
+    try:
+        g.set_mdagm_kernel(0)
+    except hq.HqmcError:
+        g.set_mdagm_kernel(3)
+    for fused in (False, True):
+        g.set_cg_fusion(fused)
+        x1 = g.cg_solve(v, 0.0, 64)[0].clone()
+        x2 = g.cg_solve(v, 0.0, 64)[0]
+        assert torch.equal(x1, x2), fused
+    g.close()
