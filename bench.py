@@ -343,9 +343,10 @@ def run_solve(args):
     from paper_2508_16298_b200 import hqmc, inputs
     c = inputs.CONFIGS[args.config]
     L, Ntau = c["L"], c["Ntau"]
-    theta = inputs.make_theta(args.config)
+    theta = inputs.theta_paper_regime(L, Ntau, c["seed"]) if args.theta == "paper" else inputs.make_theta(args.config)
     eta = inputs.complex_gaussian((Ntau, L, L), c["seed"])
-    out = {"mode": "solve", "config": args.config, "L": L, "Ntau": Ntau, "tol": args.tol, "theta": c["theta"]}
+    out = {"mode": "solve", "config": args.config, "L": L, "Ntau": Ntau, "tol": args.tol,
+           "theta": "paper regime (c_tau=80, K=1 heat bath, cold start)" if args.theta == "paper" else c["theta"]}
     for W in (6, 0):
         g = hqmc.HQMC(L, Ntau, W=W)
         g.set_theta(torch.from_numpy(theta).cuda())
@@ -404,6 +405,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--mode", default="step", choices=["step", "solve"], help="solve: one full PCG solve to --tol (not the timed metric)")
     ap.add_argument("--tol", type=float, default=1e-10)
+    ap.add_argument("--theta", default="config", choices=["config", "paper"], help="solve mode: the config's field or a paper-regime field")
     ap.add_argument("--max-iter", type=int, default=3000000)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":

@@ -74,9 +74,10 @@ def bench_vectors(n: int, L: int, Ntau: int, seed: int) -> np.ndarray:
 # Heat bath for the pure-gauge Wilson weight exp(+beta * sum_plaq cos(a_plaq)) on the (2+1)d
 # lattice with temporal links fixed to 0 (BASELINE.json configs 2 and 5).
 # ------------------------------------------------------------------------------------------------
-def _staple_sum(a: np.ndarray, mu: int) -> np.ndarray:
-    """sum_k exp(+i c_k) over the 4 plaquettes containing each mu-link, where the plaquette angle
-    is (a_link + c_k).  a has shape [Ntau][2][L][L] (axes tau, mu, y, x)."""
+def _staple_sum(a: np.ndarray, mu: int, w_space: float = 1.0, w_time: float = 1.0) -> np.ndarray:
+    """sum_k w_k exp(+i c_k) over the 4 plaquettes containing each mu-link, where the plaquette angle
+    is (a_link + c_k); w_k = w_space for the two spatial plaquettes, w_time for the two temporal ones.
+    a has shape [Ntau][2][L][L] (axes tau, mu, y, x)."""
     ax, ay = a[:, 0], a[:, 1]
     if mu == 0:
         # plaquette at s:      +ax(s) + ay(s+x) - ax(s+y) - ay(s)
@@ -93,11 +94,11 @@ def _staple_sum(a: np.ndarray, mu: int) -> np.ndarray:
     # temporal plaquettes: angle = a(tau+1) - a(tau) and a(tau) - a(tau-1)
     c_tp = -np.roll(link, -1, axis=0)
     c_tm = -np.roll(link, 1, axis=0)
-    return np.exp(1j * c_up) + np.exp(1j * c_dn) + np.exp(1j * c_tp) + np.exp(1j * c_tm)
+    return w_space * (np.exp(1j * c_up) + np.exp(1j * c_dn)) + w_time * (np.exp(1j * c_tp) + np.exp(1j * c_tm))
 
 
 def heatbath_theta(L: int, Ntau: int, seed: int, beta: float = 1.0, sweeps: int = 10,
-                   add_pi_flux: bool = True) -> np.ndarray:
+                   add_pi_flux: bool = True, beta_time: float | None = None, cold_start: bool = False) -> np.ndarray:
     """Hot start U[-pi,pi) then `sweeps` von-Mises heat-bath sweeps at coupling beta = 1/g^2.
 
     Each link's conditional density is prop. to exp(beta * Re[e^{i a} * S]) with S = sum_k e^{i c_k},
@@ -107,7 +108,8 @@ def heatbath_theta(L: int, Ntau: int, seed: int, beta: float = 1.0, sweeps: int 
     """
     assert L % 2 == 0 and Ntau % 2 == 0
     g = rng(seed, STREAM_HEATBATH)
-    a = g.uniform(-np.pi, np.pi, (Ntau, 2, L, L))
+    bt = beta if beta_time is None else beta_time       # separate temporal coupling (paper regime: c_tau = 1/(J dtau^2) = 80, K = 1)
+    a = np.zeros((Ntau, 2, L, L)) if cold_start else g.uniform(-np.pi, np.pi, (Ntau, 2, L, L))
     tau = np.arange(Ntau)[:, None, None]
     yy = np.arange(L)[None, :, None]
     xx = np.arange(L)[None, None, :]
@@ -115,9 +117,9 @@ def heatbath_theta(L: int, Ntau: int, seed: int, beta: float = 1.0, sweeps: int 
         for mu in (0, 1):
             par = (yy + tau + 0 * xx) % 2 if mu == 0 else (xx + tau + 0 * yy) % 2
             for colour in (0, 1):
-                S = _staple_sum(a, mu)
+                S = _staple_sum(a, mu, beta, bt)
                 mask = par == colour
-                kappa = beta * np.abs(S[mask])
+                kappa = np.abs(S[mask])
                 centre = -np.angle(S[mask])
                 a[:, mu][mask] = g.vonmises(centre, kappa)
     if add_pi_flux:
@@ -138,3 +140,10 @@ def make_theta(cfg: int) -> np.ndarray:
     if c["theta"] == "uniform":
         return theta_uniform(c["L"], c["Ntau"], c["seed"])
     return heatbath_theta(c["L"], c["Ntau"], c["seed"])
+
+
+def theta_paper_regime(L: int, Ntau: int, seed: int, J: float = 1.25, K: float = 1.0, dtau: float = 0.1, sweeps: int = 50) -> np.ndarray:
+    """A field typical of the paper's own simulations (J = 1.25, K = 1, dtau = 0.1, so the temporal
+    coupling is c_tau = 1/(J dtau^2) = 80): heat bath of the pure-gauge part of the compact action from a
+    cold start, theta = a + A_pi.  Smooth in tau, which is the regime the banded preconditioner was built for."""
+    return heatbath_theta(L, Ntau, seed, beta=K, sweeps=sweeps, beta_time=1.0 / (J * dtau * dtau), cold_start=True)
