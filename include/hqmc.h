@@ -111,6 +111,15 @@ int hqmc_leapfrog_trajectory(hqmc_ctx *ctx, double *d_theta, double *d_p, const 
                              double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
                              long long *cg_iters_out);
 
+/* One HQMC update, steps (i)-(iv) of PAPER.md:185-201.  The random numbers are inputs (d_eta complex Gaussian with
+ * <|eta|^2> = 1, d_p Gaussian with variance 1/2, u uniform in [0,1); reading C6), so the caller owns the generator:
+ *   phi = M^+(theta) eta;  leapfrog trajectory of nsteps steps (as hqmc_leapfrog_trajectory);
+ *   accepted iff u < min(1, exp(H0 - H1)) (Eq.15); on rejection d_theta is restored.
+ * d_theta: in/out; d_p: in/out (holds the final momenta whatever the decision).  *accepted_out: 1 or 0. */
+int hqmc_hqmc_step(hqmc_ctx *ctx, double *d_theta, double *d_p, const void *d_eta, double u, int nsteps, double eps,
+                   double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out, int *accepted_out,
+                   long long *cg_iters_out);
+
 /* HOST-buffer variants (pageable or pinned host memory; the copies run inside the call on the
  * context's stream and the call returns after the result has landed in h_out / h_x). */
 int hqmc_apply_MdagM_host(hqmc_ctx *ctx, const void *h_in, void *h_out);

@@ -390,3 +390,29 @@ long orc_trajectory(const orc_params *P, double *theta, double *p, const cplx *p
     free(X); free(gF); free(gB);
     return iters;
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * One HQMC update, steps (i)-(iv) of PAPER.md:185-201 (NEXT-1 of SURVEY.md 8f).  The random numbers are INPUTS
+ * (eta complex Gaussian, p Gaussian, u uniform in [0,1)), so that oracle and GPU consume identical draws:
+ *   (i)   phi = M^+(theta_0) eta                                   (reading C6)
+ *   (ii)  leapfrog trajectory (theta_0, p_0) -> (theta_t, p_t)      (Eq.13-16)
+ *   (iii) accept with probability r = min(1, exp(H_0 - H_t))        (Eq.15): accepted iff u < r
+ *   (iv)  on rejection theta stays theta_0 (p is discarded either way: it is redrawn next update)
+ * theta, p updated in place (p holds p_t afterwards, whatever the decision).  Returns 1 if accepted, else 0.
+ * ------------------------------------------------------------------------------------------- */
+int orc_hqmc_step(const orc_params *P, double *theta, double *p, const cplx *eta, double u, int nsteps, double eps,
+                  double cg_tol, long cg_max_iter, double *H0, double *H1, long *iters_out) {
+    const size_t N = (size_t)P->Ntau * P->L * P->L, NB = 2 * N;
+    cplx *phi = (cplx *)malloc(sizeof(cplx) * N);
+    double *theta0 = (double *)malloc(sizeof(double) * NB);
+    memcpy(theta0, theta, sizeof(double) * NB);
+    orc_apply_Mdag(P, theta, eta, phi);
+    long it = orc_trajectory(P, theta, p, phi, nsteps, eps, cg_tol, cg_max_iter, H0, H1, NULL);
+    if (iters_out) *iters_out = it;
+    double r = exp(*H0 - *H1);
+    if (r > 1.0) r = 1.0;
+    int accepted = (u < r) ? 1 : 0;
+    if (!accepted) memcpy(theta, theta0, sizeof(double) * NB);
+    free(phi); free(theta0);
+    return accepted;
+}

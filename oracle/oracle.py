@@ -43,6 +43,7 @@ def lib():
         _lib.orc_sum_p2.restype = C.c_double
         _lib.orc_max_threads.restype = C.c_int
         _lib.orc_get_threads.restype = C.c_int
+        _lib.orc_hqmc_step.restype = C.c_int
     return _lib
 
 
@@ -178,3 +179,14 @@ class Oracle:
                                   C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_long(cg_max_iter),
                                   C.byref(H0), C.byref(H1), parts.ctypes.data_as(C.c_void_p))
         return dict(theta=th, p=pp, H0=H0.value, H1=H1.value, cg_iters=int(it), parts=parts)
+
+    def hqmc_step(self, theta, p, eta, u: float, nsteps: int, eps: float, cg_tol: float = 1e-13, cg_max_iter: int = 1000000):
+        """One HQMC update -> dict(theta, p, H0, H1, accepted, cg_iters).  Inputs are not modified."""
+        th = np.array(theta, dtype=np.float64, order="C").copy()
+        pp = np.array(p, dtype=np.float64, order="C").copy()
+        e, ep = _c(np.reshape(eta, -1))
+        H0, H1, it = C.c_double(0), C.c_double(0), C.c_long(0)
+        acc = lib().orc_hqmc_step(self._p, th.ctypes.data_as(C.c_void_p), pp.ctypes.data_as(C.c_void_p), ep, C.c_double(u),
+                                  C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_long(cg_max_iter), C.byref(H0),
+                                  C.byref(H1), C.byref(it))
+        return dict(theta=th, p=pp, H0=H0.value, H1=H1.value, accepted=bool(acc), cg_iters=int(it.value))

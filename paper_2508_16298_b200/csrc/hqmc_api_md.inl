@@ -86,6 +86,32 @@ extern "C" int hqmc_leapfrog_trajectory(hqmc_ctx *c, double *d_theta, double *d_
     return noconv ? HQMC_ENOCONV : HQMC_OK;
 }
 
+extern "C" int hqmc_hqmc_step(hqmc_ctx *c, double *d_theta, double *d_p, const void *d_eta, double u, int nsteps, double eps,
+                              double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out, int *accepted_out,
+                              long long *cg_iters_out) {
+    if (!c || !aligned16(d_theta) || !aligned16(d_p) || !aligned16(d_eta) || nsteps < 0 || cg_max_iter < 0) return HQMC_EINVAL;
+    if (d_theta == c->d_force || d_theta == c->d_theta) return HQMC_EINVAL;      // d_force keeps theta_0 for the rejection
+    const size_t tb = sizeof(double) * 2 * c->N;
+    CUDA_TRY(cudaMemcpyAsync(c->d_force, d_theta, tb, cudaMemcpyDeviceToDevice, c->stream));
+    HQ_TRY(hqmc_set_theta(c, d_theta));
+    HQ_TRY(hqmc_apply_Mdag(c, d_eta, c->d_phi));                                 // (i) pseudofermion refresh
+    double H0 = 0.0, H1 = 0.0;
+    int s = hqmc_leapfrog_trajectory(c, d_theta, d_p, c->d_phi, nsteps, eps, cg_tol, cg_max_iter, &H0, &H1, cg_iters_out);   // (ii)
+    if (s != HQMC_OK && s != HQMC_ENOCONV) return s;
+    double r = std::exp(H0 - H1);
+    if (r > 1.0) r = 1.0;
+    const int acc = (u < r) ? 1 : 0;                                             // (iii)
+    if (!acc) {                                                                  // (iv)
+        CUDA_TRY(cudaMemcpyAsync(d_theta, c->d_force, tb, cudaMemcpyDeviceToDevice, c->stream));
+        CUDA_TRY(cudaStreamSynchronize(c->stream));
+        c->theta_set = false;                                                    // the context's phase tables belong to theta_t
+    }
+    if (H0_out) *H0_out = H0;
+    if (H1_out) *H1_out = H1;
+    if (accepted_out) *accepted_out = acc;
+    return s;
+}
+
 // ---------------------------------------------------------------------------------------------------
 // host-buffer variants: H2D copies, compute, D2H copies, all on the context's stream
 // ---------------------------------------------------------------------------------------------------

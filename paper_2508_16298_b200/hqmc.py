@@ -23,7 +23,7 @@ KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
-    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_fusion", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
@@ -185,6 +185,15 @@ class HQMC:
                                                  C.c_longlong(cg_max_iter), C.byref(H0), C.byref(H1), C.byref(it)),
                    allow_noconv=True)
         return dict(H0=H0.value, H1=H1.value, cg_iters=it.value, converged=(s == HQMC_OK))
+
+    def hqmc_step(self, theta, p, eta, u, nsteps, eps, cg_tol=1e-10, cg_max_iter=1000000):
+        """One HQMC update, in place on theta (restored on rejection) and p.
+        -> dict(H0, H1, accepted, cg_iters, converged)."""
+        H0, H1, it, acc = C.c_double(0), C.c_double(0), C.c_longlong(0), C.c_int(0)
+        s = _check(_lib.hqmc_hqmc_step(self._ctx, _ptr(self._field(theta)), _ptr(self._field(p)), _ptr(self._vec(eta)),
+                                       C.c_double(u), C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter),
+                                       C.byref(H0), C.byref(H1), C.byref(acc), C.byref(it)), allow_noconv=True)
+        return dict(H0=H0.value, H1=H1.value, accepted=bool(acc.value), cg_iters=it.value, converged=(s == HQMC_OK))
 
     # ---- host-buffer entry points (numpy arrays, pageable or pinned) ----------------------------
     def apply_MdagM_host(self, h_in: np.ndarray, h_out: np.ndarray):

@@ -282,3 +282,28 @@ def test_kernels_are_deterministic_run_to_run(hq, L, Nt):
         x2 = g.cg_solve(v, 0.0, 64)[0]
         assert torch.equal(x1, x2), fused
     g.close()
+
+
+@pytest.mark.parametrize("L,Nt,seed,u,cpl,want", [(4, 8, 0, 0.3, 0.0, True), (4, 8, 0, 0.99, 0.0, False), (6, 10, 1, 0.5, 0.0, True),
+                                                   (6, 10, 1, 0.99, 0.0, False), (6, 10, 1, 0.99, 1.0, True)])
+def test_hqmc_step_accept_and_reject(hq, L, Nt, seed, u, cpl, want):
+    """NEXT-1: one full HQMC update (refresh, trajectory, Metropolis) against the oracle with the same
+    draws.  With c_tau = K = 0 and eps = 0.15, dH = +0.07 (acceptance 0.93): u = 0.99 is a rejection and theta must come
+    back bit for bit; with c_tau = K = 1, dH < 0 and every u accepts."""
+    o, g, theta = setup(hq, L, Nt, seed, c_tau=cpl, K=cpl)
+    eta = inputs.complex_gaussian((Nt, L, L), seed)
+    p = inputs.momenta(L, Nt, seed)
+    ref = o.hqmc_step(theta, p, eta, u, 6, 0.15, cg_tol=1e-13)
+    dth, dp = dev(theta), dev(p)
+    r = g.hqmc_step(dth, dp, dev(eta), u, 6, 0.15, cg_tol=1e-13)
+    assert r["converged"] and r["accepted"] == ref["accepted"] == want
+    assert abs(r["H0"] - ref["H0"]) <= 1e-8 and abs((r["H1"] - r["H0"]) - (ref["H1"] - ref["H0"])) <= 1e-8
+    if ref["accepted"]:
+        assert np.abs(dth.cpu().numpy() - ref["theta"]).max() <= 1e-10
+    else:
+        assert np.array_equal(dth.cpu().numpy(), theta)
+    assert np.abs(dp.cpu().numpy() - ref["p"]).max() <= 1e-10
+    v = inputs.complex_gaussian((Nt, L, L), seed + 5, inputs.STREAM_VEC)      # the context is usable afterwards
+    g.set_theta(dth)
+    assert rel(g.apply_MdagM(dev(v)).cpu().numpy(), o.apply_MdagM(dth.cpu().numpy(), v)) <= 1e-12
+    g.close()

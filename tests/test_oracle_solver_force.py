@@ -154,3 +154,23 @@ def test_heatbath_generator_plaquette():
     assert 0.446 < ps < 0.50 and 0.446 < pt < 0.50
     th = inputs.heatbath_theta(12, 120, 1)
     assert abs(inputs.mean_plaquettes(th)[0] + ps) < 1e-12   # + A_pi flips the sign of cos(curl)
+
+
+def test_hqmc_step_metropolis_rule():
+    """orc_hqmc_step: H0 = S_B + sum p^2 + eta^+ eta exactly (phi = M^+ eta), the decision is
+    u < min(1, e^{H0-H1}) (Eq.15), theta is restored on rejection and equals the trajectory's end point on acceptance."""
+    L, Nt = 4, 8
+    theta = inputs.theta_uniform(L, Nt, 0)
+    p = inputs.momenta(L, Nt, 0)
+    eta = inputs.complex_gaussian((Nt, L, L), 0)
+    o = orc.Oracle(L, Nt, c_tau=0.0, K=0.0)     # (with c_tau = K = 1 this far-from-equilibrium field always has dH < 0)
+    phi = o.apply_Mdag(theta, eta)
+    t = o.trajectory(theta, p, phi, 6, 0.15)
+    r_acc = min(1.0, np.exp(t["H0"] - t["H1"]))
+    assert abs(t["H0"] - (o.action_boson(theta) + o.sum_p2(p) + np.vdot(eta, eta).real)) < 1e-9
+    assert 0.0 < r_acc < 1.0            # dH = +0.067 here, so both branches are reachable
+    for u, want in ((r_acc - 1e-9, True), (r_acc + 1e-9, False), (0.0, True)):
+        s = o.hqmc_step(theta, p, eta, u, 6, 0.15)
+        assert s["accepted"] is want and s["H0"] == t["H0"] and s["H1"] == t["H1"]
+        assert np.array_equal(s["theta"], t["theta"] if want else theta)
+        assert np.array_equal(s["p"], t["p"])
