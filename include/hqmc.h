@@ -145,7 +145,9 @@ int hqmc_get_kernel_stats(hqmc_ctx *ctx, int which, long long *launches_out, dou
  * with the slices dealt out evenly).  hqmc_set_mdagm_kernel: 0 = streaming kernel (TMA bulk copies, packed link
  * phases; default where its staging buffers fit one SM: L <= 48 in complex128), 1 = register-only kernel,
  * 2 = warp-specialised strip-decoupled streaming kernel, 3 = cluster kernel (the slice split over 2/4/8 SMs with
- * distributed shared memory; default where one SM cannot hold the slice, e.g. L = 64 in complex128). */
+ * distributed shared memory; default where one SM cannot hold the slice, e.g. L = 64 in complex128), 4 = streaming
+ * kernel that sweeps its time run backwards (fewer live registers, third v buffer), 5 = the same with the halo
+ * product handed over between neighbouring CTAs instead of recomputed. */
 int hqmc_set_time_tile(hqmc_ctx *ctx, int slices_per_cta);
 int hqmc_set_mdagm_kernel(hqmc_ctx *ctx, int which);
 /* Preconditioner kernel for W = 1..6: n > 0: TMA-tiled kernel, runs of n slices per CTA; n < 0: register-ring

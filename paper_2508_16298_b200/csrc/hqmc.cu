@@ -69,6 +69,12 @@ template <typename T> static int set_attrs(hqmc_ctx *c) {
             CUDA_TRY(cudaFuncSetAttribute(k_mdagm_stream<T, false>, attr, (int)c->stream_smem));
             CUDA_TRY(cudaFuncSetAttribute(k_mdagm_stream<T, true>, attr, (int)c->stream_smem));
         }
+        if (c->use_back) {
+            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, false, false>, attr, (int)c->back_smem));
+            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, true, false>, attr, (int)c->back_smem));
+            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, false, true>, attr, (int)c->back_smem));
+            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, true, true>, attr, (int)c->back_smem));
+        }
         if (c->use_ws) {
             CUDA_TRY(cudaFuncSetAttribute(k_mdagm_ws<T, false>, attr, (int)c->ws_smem));
             CUDA_TRY(cudaFuncSetAttribute(k_mdagm_ws<T, true>, attr, (int)c->ws_smem));
@@ -122,6 +128,14 @@ template <typename T> static int do_mdagm_stream(hqmc_ctx *c, const void *in, vo
     typedef typename PhasePack<T>::word W;
     int G = c->time_tile > 0 ? (c->g.Nt + c->time_tile - 1) / c->time_tile : (c->g.Nt < c->n_sm ? c->g.Nt : c->n_sm);
     c->grid_mdagm = G;
+    if (c->use_back && c->back_on) {
+        auto go = [&](auto kern, double *part) -> int {
+            return launch(c, HQMC_K_MDAGM, kern, dim3(G), dim3(c->cfg.threads), c->back_smem, c->g, (const W *)c->d_packed,
+                          (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, part, st, (T2 *)c->d_halo, c->d_flags);
+        };
+        if (c->back_coop) return dot ? go(k_mdagm_back<T, true, true>, c->d_part_dOd) : go(k_mdagm_back<T, false, true>, (double *)nullptr);
+        return dot ? go(k_mdagm_back<T, true, false>, c->d_part_dOd) : go(k_mdagm_back<T, false, false>, (double *)nullptr);
+    }
     if (c->use_ws && c->ws_on) {
         if (dot)
             return launch(c, HQMC_K_MDAGM, k_mdagm_ws<T, true>, dim3(G), dim3(c->cfg.threads + 32), c->ws_smem, c->g,

@@ -106,6 +106,9 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
                                               : WsSmem<float>(c->g.Vs, c->cfg.threads, h, ws_ns).total;
         c->use_ws = c->use_stream && c->cfg.threads + 32 <= 608 && c->ws_smem <= (size_t)prop.sharedMemPerBlockOptin;
         c->ws_on = false;   // measured slower than k_mdagm_stream (profiles/): kept selectable
+        c->back_smem = (prm->prec == HQMC_C128) ? BackSmem<double>(c->g.Vs, c->cfg.threads).total : BackSmem<float>(c->g.Vs, c->cfg.threads).total;
+        c->use_back = c->use_stream && c->back_smem <= (size_t)prop.sharedMemPerBlockOptin;
+        c->back_on = c->use_back; c->back_coop = false;   // default: backward sweep, halo recomputed (hand-over measured slower)
         // cluster kernel: the slice split over R SMs (smallest R whose strip fits one SM's threads and shared memory)
         c->use_cluster = false; c->cluster_on = false; c->cl_R = 0;
         for (int R = 2; R <= 8 && !c->use_cluster; R *= 2) {
@@ -117,6 +120,11 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
             }
         }
         c->cluster_on = c->use_cluster && !c->use_stream;      // default only where one SM cannot hold the slice
+    }
+    if (c->use_back) {
+        ALLOC(c->d_halo, c->N * c->esz);
+        ALLOC(c->d_flags, sizeof(unsigned) * HQMC_MAX_PART);
+        cudaMemset(c->d_flags, 0, sizeof(unsigned) * HQMC_MAX_PART);
     }
     if (c->use_stream || c->use_cluster) {
         ALLOC(c->d_packed, 2 * c->N * 8);
@@ -159,7 +167,7 @@ extern "C" int hqmc_destroy(hqmc_ctx *c) {
     if (c->cg_graph) cudaGraphExecDestroy(c->cg_graph);
     for (auto &ep : c->pending) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (auto &ep : c->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-    void *ptrs[] = {c->d_r2, c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
+    void *ptrs[] = {c->d_halo, c->d_flags, c->d_r2, c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
                     c->d_part_rr, c->d_part_rz[0], c->d_part_rz[1], c->d_part_misc, c->d_state, c->d_scal};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (c->h_state) cudaFreeHost(c->h_state);
@@ -268,10 +276,13 @@ extern "C" int hqmc_set_cg_fusion(hqmc_ctx *c, int on) {
     return HQMC_OK;
 }
 extern "C" int hqmc_set_mdagm_kernel(hqmc_ctx *c, int which) {
-    if (!c || which < 0 || which > 3) return HQMC_EINVAL;
-    if ((which == 0 && !c->use_stream) || (which == 2 && !c->use_ws) || (which == 3 && !c->use_cluster)) return HQMC_EINVAL;
-    c->stream_on = (which == 0 || which == 2);
+    if (!c || which < 0 || which > 5) return HQMC_EINVAL;
+    if ((which == 0 && !c->use_stream) || (which == 2 && !c->use_ws) || (which == 3 && !c->use_cluster) || (which >= 4 && !c->use_back))
+        return HQMC_EINVAL;
+    c->stream_on = (which == 0 || which == 2 || which >= 4);
     c->ws_on = (which == 2);
+    c->back_on = (which >= 4);
+    c->back_coop = (which == 5);
     c->cluster_on = (which == 3);
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     return hqmc_set_time_tile(c, 0);

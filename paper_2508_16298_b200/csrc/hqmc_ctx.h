@@ -16,6 +16,7 @@
 #include "mdagm_stream.cuh"
 #include "mdagm_ws.cuh"
 #include "mdagm_cluster.cuh"
+#include "mdagm_back.cuh"
 #include "precond_tma.cuh"
 
 namespace hqmc {
@@ -62,6 +63,8 @@ struct hqmc_ctx {
     double2 *d_tab;      // [2][1024] tanh(a) e^{i k delta} (half step, full step)
     bool stream_on;      // runtime switch (hqmc_set_mdagm_kernel): a streaming kernel is selected
     bool use_ws, ws_on;  // warp-specialised strip kernel usable / selected
+    bool back_coop; void *d_halo; unsigned *d_flags;   // halo hand-over between CTAs (k_mdagm_back<COOP>)
+    bool use_back, back_on; size_t back_smem;   // backward-sweep streaming kernel usable / selected
     bool use_cluster, cluster_on;   // cluster kernel (slice split over R SMs) usable / selected
     int cl_R, cl_threads; size_t cl_smem;
     size_t ws_smem;

@@ -48,12 +48,12 @@ def test_M_Mdag_MdagM(hq, L, Nt, seed):
     assert rel(g.apply_Mdag(dv).cpu().numpy(), o.apply_Mdag(theta, v)) <= 1e-12
     ref = o.apply_MdagM(theta, v)
     assert rel(g.apply_MdagM(dv).cpu().numpy(), ref) <= 1e-12
-    for which in (3, 2, 0, 1):        # 3: cluster (DSMEM) kernel, 2: warp-specialised strips, 0: streaming (TMA) kernel, 1: register-only
+    for which in (5, 4, 3, 2, 0, 1):  # 5 / 4: backward streaming kernel with / without halo hand-over, 3: cluster (DSMEM) kernel, 2: warp-specialised strips, 0: streaming (TMA) kernel, 1: register-only
         try:
             g.set_mdagm_kernel(which)
         except hq.HqmcError:      # not available for this lattice: streaming kernels need the slice on one SM (L <= 48),
             assert which != 1      # the cluster kernel an even number of block-rows and a strip that fits one SM
-            assert (which in (0, 2) and L > 48) or (which == 3 and ((L // 2) % 2 or L > 96))
+            assert (which in (0, 2, 4, 5) and L > 48) or (which == 3 and ((L // 2) % 2 or L > 96))
             continue
         for tt in (0, 1, 2, 3, Nt):   # default split and every time-tile shape incl. ragged last tile and one-CTA-for-all
             g.set_time_tile(tt)
@@ -262,7 +262,7 @@ def test_kernels_are_deterministic_run_to_run(hq, L, Nt):
     g = hq.HQMC(L, Nt)
     g.set_theta(dev(theta))
     v = dev(inputs.complex_gaussian((Nt, L, L), 11, inputs.STREAM_VEC))
-    for which in (0, 2, 3, 1):
+    for which in (0, 2, 3, 4, 5, 1):
         try:
             g.set_mdagm_kernel(which)
         except hq.HqmcError:
