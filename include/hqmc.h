@@ -156,6 +156,9 @@ int hqmc_set_precond_tile(hqmc_ctx *ctx, int slices_per_run);
 /* PCG vector kernels: 1 = fused residual-update + preconditioner and fused x/d update where the
  * TMA-tiled preconditioner applies (3 kernels per iteration); 0 (default) = the four separate kernels. */
 int hqmc_set_cg_fusion(hqmc_ctx *ctx, int on);
+/* Programmatic dependent launch of the PCG kernels (kernel k+1 is launched while kernel k runs and waits on-device
+ * for its completion before reading its output). */
+int hqmc_set_pdl(hqmc_ctx *ctx, int on);
 /* TIMING ONLY: bit k of mask set = kernels of class HQMC_K_<k> are not launched (leave-one-out timing of a kernel
  * inside the graph-replayed PCG iteration; the numerical results are then meaningless).  0 restores normal operation. */
 int hqmc_set_debug_skip(hqmc_ctx *ctx, unsigned mask);

@@ -35,6 +35,7 @@ __global__ void k_cg_axpy(size_t N, typename Cx<T>::type *__restrict__ x, typena
                           const double *__restrict__ part_rz, int n_rz, const double *__restrict__ part_dOd, int n_dOd,
                           double *__restrict__ part_rr, const CgState *__restrict__ st) {
     typedef typename Cx<T>::type T2;
+    pdl_wait();
     if (*(volatile const int *)&st->done) return;
     __shared__ double red[34];
     const double rz = cta_sum_partials(part_rz, n_rz, threadIdx.x, blockDim.x, red);
@@ -48,6 +49,7 @@ __global__ void k_cg_axpy(size_t N, typename Cx<T>::type *__restrict__ x, typena
         x[i] = xi; r[i] = ri;
         acc += (double)ri.x * (double)ri.x + (double)ri.y * (double)ri.y;
     }
+    pdl_launch_dependents();
     double s = block_sum(acc, red);
     if (threadIdx.x == 0) part_rr[blockIdx.x] = s;
 }
@@ -184,6 +186,7 @@ __global__ void k_cg_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, con
                              const double *__restrict__ part_new, const double *__restrict__ part_old, int n,
                              int first, const CgState *__restrict__ st) {
     typedef typename Cx<T>::type T2;
+    pdl_wait();
     if (*(volatile const int *)&st->done) return;
     __shared__ double red[34];
     double bt = 0.0;
@@ -198,6 +201,7 @@ __global__ void k_cg_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, con
         if (!first) { T2 di = d[i]; zi.x = fma(beta, di.x, zi.x); zi.y = fma(beta, di.y, zi.y); }
         d[i] = zi;
     }
+    pdl_launch_dependents();
 }
 
 // Generic deterministic reductions for the energies (Eq.12).

@@ -24,6 +24,8 @@ static int drain_events(hqmc_ctx *c) {
 
 template <typename... KArgs, typename... Args>
 static int launch(hqmc_ctx *c, int kclass, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args) {
+    const bool use_pdl = c->pdl && c->pdl_next;
+    c->pdl_next = false;
     if (c->skip_mask & (1u << kclass)) return HQMC_OK;   // leave-one-out timing (results are then meaningless)
     if (c->capturing) c->graph_nodes[kclass]++; else c->launches[kclass]++;
     const bool prof = c->profiling && !c->capturing;
@@ -35,8 +37,21 @@ static int launch(hqmc_ctx *c, int kclass, void (*kernel)(KArgs...), dim3 grid, 
         ep.kclass = kclass;
         CUDA_TRY(cudaEventRecord(ep.a, c->stream));
     }
-    kernel<<<grid, block, smem, c->stream>>>(static_cast<KArgs>(args)...);
-    CUDA_TRY(cudaGetLastError());
+    if (use_pdl) {
+        // programmatic dependent launch: the PCG kernels call griddepcontrol.launch_dependents at their top and
+        // griddepcontrol.wait before touching anything the previous kernel wrote, so the launch latency of kernel k+1
+        // (and, for M^+M, its barrier set-up and table fetch) hides under kernel k instead of adding to the iteration
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        CUDA_TRY(cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...));
+    } else {
+        kernel<<<grid, block, smem, c->stream>>>(static_cast<KArgs>(args)...);
+        CUDA_TRY(cudaGetLastError());
+    }
     if (prof) { CUDA_TRY(cudaEventRecord(ep.b, c->stream)); c->pending.push_back(ep); }
     return HQMC_OK;
 }
@@ -130,6 +145,7 @@ template <typename T> static int do_mdagm_stream(hqmc_ctx *c, const void *in, vo
     c->grid_mdagm = G;
     if (c->use_back && c->back_on) {
         auto go = [&](auto kern, double *part) -> int {
+            c->pdl_next = true;                       // k_mdagm_back calls griddepcontrol.wait
             return launch(c, HQMC_K_MDAGM, kern, dim3(G), dim3(c->cfg.threads), c->back_smem, c->g, (const W *)c->d_packed,
                           (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, part, st, (T2 *)c->d_halo, c->d_flags);
         };
@@ -262,6 +278,7 @@ template <typename T> static int do_cg_rz(hqmc_ctx *c, const void *rin, void *ro
 template <typename T, int W> static int launch_precond_win(hqmc_ctx *c, const void *in, void *out, double *part_rz, int mode) {
     typedef typename Cx<T>::type T2;
     if (c->pc_kind == 2) {
+        c->pdl_next = true;
         CUDA_TRY(cudaFuncSetAttribute(k_precond_tma<T, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->pc_smem));
         return launch(c, HQMC_K_PRECOND, k_precond_tma<T, W>, dim3(c->pc_gx, c->pc_gy), dim3(128), c->pc_smem, c->g, c->taps,
                       (const T2 *)in, (T2 *)out, part_rz, (const double *)c->d_part_rr, c->grid_ew, c->d_state, mode, c->pc_tile);

@@ -19,10 +19,12 @@ template <typename T> static int cg_iteration(hqmc_ctx *c, void *x, int par) {
                       (const double *)c->d_part_rz[par], (const double *)c->d_part_rz[par ^ 1], c->n_part_f,
                       (const double *)c->d_part_dOd, c->grid_mdagm, (const double *)c->d_part_rr, c->d_state);
     }
+    c->pdl_next = true;
     HQ_TRY(launch(c, HQMC_K_AXPY, k_cg_axpy<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_r, (const T2 *)c->d_d,
                   (const T2 *)c->d_Od, (const double *)c->d_part_rz[par], c->n_part_rz, (const double *)c->d_part_dOd,
                   c->grid_mdagm, c->d_part_rr, (const CgState *)c->d_state));
     HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[par ^ 1], 2));
+    c->pdl_next = true;
     HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)c->d_z,
                   (const double *)c->d_part_rz[par ^ 1], (const double *)c->d_part_rz[par], c->n_part_rz, 0,
                   (const CgState *)c->d_state));

@@ -65,7 +65,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     c->own_stream = (cuda_stream == nullptr);
     c->stream = (cudaStream_t)cuda_stream;
     c->cg_graph = nullptr; c->cg_graph_x = nullptr; c->cg_graph_tile = 0; c->cg_graph_fused = false; c->cg_chunk = 32;
-    c->profiling = false; c->capturing = false; c->theta_set = false; c->skip_mask = 0; c->cg_fused = false;
+    c->profiling = false; c->capturing = false; c->theta_set = false; c->skip_mask = 0; c->cg_fused = false; c->pdl = false; c->pdl_next = false;
     c->fused_allowed = false;   // fused PCG vector kernels measured no faster at L=48: opt-in
     for (int i = 0; i < HQMC_K_COUNT; ++i) { c->launches[i] = 0; c->graph_nodes[i] = 0; c->ms[i] = 0.0; }
     int st = HQMC_OK;
@@ -265,6 +265,12 @@ extern "C" int hqmc_set_precond_tile(hqmc_ctx *c, int slices_per_run) {
 extern "C" int hqmc_set_debug_skip(hqmc_ctx *c, unsigned mask) {
     if (!c) return HQMC_EINVAL;
     c->skip_mask = mask;
+    if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+    return HQMC_OK;
+}
+extern "C" int hqmc_set_pdl(hqmc_ctx *c, int on) {
+    if (!c) return HQMC_EINVAL;
+    c->pdl = on != 0;
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     return HQMC_OK;
 }

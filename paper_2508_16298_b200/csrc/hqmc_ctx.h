@@ -95,6 +95,8 @@ struct hqmc_ctx {
     bool cg_graph_fused;
     int cg_chunk;            // iterations per graph launch
     // instrumentation
+    bool pdl_next;        // set by a call site whose kernel calls griddepcontrol.wait; consumed by launch()
+    bool pdl;             // programmatic dependent launch of the PCG kernels (hqmc_set_pdl)
     unsigned skip_mask;   // timing-only: kernel classes NOT launched inside the PCG iteration (hqmc_set_debug_skip)
     bool profiling;
     bool capturing;

@@ -101,7 +101,10 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_back(Geo g, const typename Pha
         mbar_init(bar_v, 1); mbar_init(bar_v + 1, 1); mbar_init(bar_v + 2, 1); mbar_init(bar_p, 1); mbar_init(bar_t, 1);
         mbar_fence_init();
         if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_TAB * sizeof(double2), bar_t);
-        load_p(1);                                      // links of slice t1 - 1
+        load_p(1);                                      // links of slice t1 - 1: do not depend on the previous kernel
+    }
+    pdl_wait();                                         // `in`, `st` and (COOP) the flags are the previous kernels' output
+    if (leader) {
         load_v(1); load_v(0);
         if (2 <= n_last_v) load_v(2);
     }
@@ -141,6 +144,7 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_back(Geo g, const typename Pha
         const int n = j + 1, t = slice_of(n), tm = slice_of(n + 1);
         const T sCt = sC_of(t), sCm = sC_of(tm);
         const bool recv = consume && (j == nsl - 1);    // last step: the halo product comes from the CTA below
+        if (j == nsl - 1) pdl_launch_dependents();      // let the next kernel's CTAs be dispatched under this CTA's tail
         // 1. q = B_t w_{t+1} / C.  First barrier: everyone is past the previous step -> thread 0 stores out_{t+1} (staged in
         //    buffer n-1) and fetches the links of slice t-1 (pbuf was decoded before the previous step's second sweep).
         //    Second barrier: that store has surely finished reading, so the same buffer can take v_{t-2} (slice n+2).

@@ -23,6 +23,7 @@ __global__ void __launch_bounds__(128) k_precond_tma(Geo g, Taps taps, const typ
     typedef typename Cx<T>::type T2;
     static_assert(W >= 1 && W <= 6, "register ring of 13 slots");
     constexpr int RING = 2 * W + 1;
+    pdl_wait();
     if (mode != 0 && *(volatile const int *)&st->done) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ double red[32];
@@ -86,6 +87,7 @@ __global__ void __launch_bounds__(128) k_precond_tma(Geo g, Taps taps, const typ
             }
         }
     }
+    pdl_launch_dependents();
     double sblk = block_sum(acc, red);
     const int bid = blockIdx.y * gridDim.x + blockIdx.x;
     if (threadIdx.x == 0 && part_rz != nullptr) part_rz[bid] = sblk;

@@ -25,7 +25,7 @@ SYMBOLS = [
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
     "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
-    "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_fusion", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
+    "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_fusion", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
 
 
@@ -128,6 +128,9 @@ class HQMC:
 
     def set_cg_fusion(self, on: bool):
         _check(_lib.hqmc_set_cg_fusion(self._ctx, C.c_int(int(on))))
+
+    def set_pdl(self, on: bool):
+        _check(_lib.hqmc_set_pdl(self._ctx, C.c_int(int(on))))
 
     def set_debug_skip(self, mask: int):
         """Timing only: do not launch the kernel classes whose bit is set (results become meaningless)."""

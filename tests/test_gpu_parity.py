@@ -281,6 +281,11 @@ def test_kernels_are_deterministic_run_to_run(hq, L, Nt):
         x1 = g.cg_solve(v, 0.0, 64)[0].clone()
         x2 = g.cg_solve(v, 0.0, 64)[0]
         assert torch.equal(x1, x2), fused
+    g.set_cg_fusion(False)
+    g.set_pdl(True)                       # programmatic dependent launch: same arithmetic, different launch overlap
+    x3 = g.cg_solve(v, 0.0, 64)[0].clone()
+    g.set_pdl(False)
+    assert torch.equal(x3, g.cg_solve(v, 0.0, 64)[0])
     g.close()
 
 
