@@ -156,8 +156,11 @@ def workload_config(args, L, Ntau, cg_iters):
                         f"step = M^+ refresh + 1 leapfrog step (2 fixed-count PCG solves, W=6 preconditioner, force, kicks, "
                         f"drift, energies)",
             "L": L, "Ntau": Ntau, "sites": L * L * Ntau, "cg_iters_per_solve": cg_iters, "precond_W": 6,
-            "l2": "step footprint (7 fermion vectors + phase table + theta, p) exceeds the 126 MB L2 at L=48; the M^+M "
-                  "kernel sweep additionally rotates 8 input/output buffer pairs"}
+            "l2": "no flush inside a step: a step is 2 x cg_iters_per_solve PCG iterations over the same vectors, and the solver "
+                  "keeps that loop's live set (r, d, Od|z, packed phases = 71 MB at L=48, x streamed evict-first) L2-resident "
+                  "on purpose -- the reuse is the algorithm's own, not a benchmark artefact; the whole step (7 fermion vectors "
+                  "+ phases + theta, p, force) exceeds the 126 MB L2, and the separate M^+M kernel sweep rotates 8 input/output "
+                  "buffer pairs (cold) next to the same-buffer (warm) figure"}
 
 
 # --------------------------------------------------------------------------------------------------
@@ -284,6 +287,12 @@ def run_gpu(args):
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": TRAFFIC_NCU.get(dom), "peak_source": peak_src, "alg_bytes_per_site": bps[dom],
                 "how": "leave-one-out CUDA-event timing of the graph-replayed fixed-count PCG solve (bench.py pcg_kernel_costs)"}
+    # the whole PCG iteration against the same peak: algorithmic bytes of all its kernels / the iteration time.  The vector
+    # kernels are served largely from L2 (their alg_GBps can exceed the HBM peak), so this is a figure of merit against the
+    # HBM-streaming model of the iteration, not a DRAM-traffic claim (in-situ DRAM bytes: profiles/).
+    it_bytes = sum(bps.values()) * N
+    roofline["iteration"] = {"alg_bytes_per_site": sum(bps.values()), "achieved": it_bytes / kern["iter_us"] / 1e3, "unit": "GB/s",
+                             "frac": it_bytes / kern["iter_us"] / 1e3 / peak}
     ms_per_step = ms / args.steps
     us_per_iter = kern["iter_us"]
     cb_dt, cb_apps, cb_threads = oracle_step_sample(L, Ntau, c["seed"], args.ref_cg_iters)

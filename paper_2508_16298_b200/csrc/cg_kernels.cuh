@@ -43,10 +43,13 @@ __global__ void k_cg_axpy(size_t N, typename Cx<T>::type *__restrict__ x, typena
     const T alpha = (T)(rz / dOd);
     double acc = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
-        T2 xi = x[i], ri = r[i], di = d[i], oi = Od[i];
+        // x is touched once per iteration: streaming (evict-first) accesses keep it from displacing r, d, Od/z and the
+        // packed phases, which then stay L2-resident between kernels
+        T2 xi = __ldcs(x + i), ri = r[i], di = d[i], oi = Od[i];
         xi.x = fma(alpha, di.x, xi.x); xi.y = fma(alpha, di.y, xi.y);
         ri.x = fma(-alpha, oi.x, ri.x); ri.y = fma(-alpha, oi.y, ri.y);
-        x[i] = xi; r[i] = ri;
+        __stcs(x + i, xi);
+        r[i] = ri;
         acc += (double)ri.x * (double)ri.x + (double)ri.y * (double)ri.y;
     }
     pdl_launch_dependents();
@@ -94,7 +97,7 @@ __global__ void k_precond(Geo g, Taps taps, const typename Cx<T>::type *__restri
         if (threadIdx.x == 0) {
             if (mode == 1) {
                 st->bb = rr; st->rr = rr; st->iters = 0;
-                st->done = (rr == 0.0 || st->max_iter <= 0) ? 1 : 0;
+                st->done = (rr == 0.0 || st->max_iter <= 0) ? 2 : 0;     // 2: finished, no iterate update pending
             } else {
                 long long it = st->iters + 1;
                 st->iters = it; st->rr = rr;
@@ -170,7 +173,7 @@ __global__ void __launch_bounds__(128) k_precond_win(Geo g, Taps taps, const typ
         if (threadIdx.x == 0) {
             if (mode == 1) {
                 st->bb = rr; st->rr = rr; st->iters = 0;
-                st->done = (rr == 0.0 || st->max_iter <= 0) ? 1 : 0;
+                st->done = (rr == 0.0 || st->max_iter <= 0) ? 2 : 0;     // 2: finished, no iterate update pending
             } else {
                 long long it = st->iters + 1;
                 st->iters = it; st->rr = rr;
@@ -200,6 +203,73 @@ __global__ void k_cg_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, con
         T2 zi = z[i];
         if (!first) { T2 di = d[i]; zi.x = fma(beta, di.x, zi.x); zi.y = fma(beta, di.y, zi.y); }
         d[i] = zi;
+    }
+    pdl_launch_dependents();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Deferred-x form of the two vector kernels (opt-in, hqmc_set_cg_fusion(2)): x_{k+1} = x_k + alpha_k d_k is applied when d_k is read anyway
+// to form d_{k+1}, so d is streamed once per iteration instead of twice (128 instead of 144 B/site for the pair):
+//   k_cg_raxpy   :  alpha = <r,z>/<d,Od>;  r -= alpha Od;  partial ||r||^2                      (48 B/site)
+//   k_cg_xdupdate:  x += alpha d;  beta = <r,z>_new/<r,z>_old;  d = z + beta d                 (80 B/site)
+// The iterate must still receive its last update when the solve stops, so `done` has three states here:
+// 0 running; 1 stop decided by the preconditioner kernel of this iteration, x update pending (k_cg_xdupdate then
+// applies x += alpha d only); 2 finished (set by the next k_cg_raxpy, or at start-up when there is nothing to do).
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void k_cg_raxpy(size_t N, typename Cx<T>::type *__restrict__ r, const typename Cx<T>::type *__restrict__ Od,
+                           const double *__restrict__ part_rz, int n_rz, const double *__restrict__ part_dOd, int n_dOd,
+                           double *__restrict__ part_rr, CgState *st) {
+    typedef typename Cx<T>::type T2;
+    pdl_wait();
+    {
+        const int done = *(volatile const int *)&st->done;
+        if (done) { if (done == 1 && blockIdx.x == 0 && threadIdx.x == 0) *(volatile int *)&st->done = 2; return; }
+    }
+    __shared__ double red[34];
+    const double rz = cta_sum_partials(part_rz, n_rz, threadIdx.x, blockDim.x, red);
+    const double dOd = cta_sum_partials(part_dOd, n_dOd, threadIdx.x, blockDim.x, red);
+    const T alpha = (T)(rz / dOd);
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        T2 ri = r[i], oi = Od[i];
+        ri.x = fma(-alpha, oi.x, ri.x); ri.y = fma(-alpha, oi.y, ri.y);
+        r[i] = ri;
+        acc += (double)ri.x * (double)ri.x + (double)ri.y * (double)ri.y;
+    }
+    pdl_launch_dependents();
+    double s = block_sum(acc, red);
+    if (threadIdx.x == 0) part_rr[blockIdx.x] = s;
+}
+
+template <typename T>
+__global__ void k_cg_xdupdate(size_t N, typename Cx<T>::type *__restrict__ x, typename Cx<T>::type *__restrict__ d,
+                              const typename Cx<T>::type *__restrict__ z, const double *__restrict__ part_rz_new,
+                              const double *__restrict__ part_rz_old, int n_rz, const double *__restrict__ part_dOd, int n_dOd,
+                              const CgState *__restrict__ st) {
+    typedef typename Cx<T>::type T2;
+    pdl_wait();
+    const int done = *(volatile const int *)&st->done;
+    if (done == 2) return;
+    __shared__ double red[34];
+    const double rz_old = cta_sum_partials(part_rz_old, n_rz, threadIdx.x, blockDim.x, red);
+    const double dOd = cta_sum_partials(part_dOd, n_dOd, threadIdx.x, blockDim.x, red);
+    const T alpha = (T)(rz_old / dOd);
+    if (done == 1) {                                  // last iteration: only the iterate is completed
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+            T2 xi = __ldcs(x + i); const T2 di = d[i];
+            xi.x = fma(alpha, di.x, xi.x); xi.y = fma(alpha, di.y, xi.y);
+            __stcs(x + i, xi);
+        }
+        return;
+    }
+    const double rz_new = cta_sum_partials(part_rz_new, n_rz, threadIdx.x, blockDim.x, red);
+    const T beta = (T)(rz_new / rz_old);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        T2 xi = __ldcs(x + i), di = d[i]; const T2 zi = z[i];
+        xi.x = fma(alpha, di.x, xi.x); xi.y = fma(alpha, di.y, xi.y);
+        di.x = fma(beta, di.x, zi.x); di.y = fma(beta, di.y, zi.y);
+        __stcs(x + i, xi); d[i] = di;
     }
     pdl_launch_dependents();
 }

@@ -238,7 +238,18 @@ static void precond_cfg(hqmc_ctx *c, int tile) {
     const int gx = (c->g.Vs + 127) / 128;
     c->pc_kind = tile < 0 ? 1 : 2;
     if (tile < 0) tile = -tile;
-    if (tile == 0) tile = 24;   // 2W = 12 halo rows re-read per run of 24 (50 %); measured best at L=48 (profiles/)
+    if (tile == 0) {
+        // Default: the shortest run whose CTAs are all resident at once (one wave). With the CG vectors L2-resident the halo
+        // re-reads are cheap and many small CTAs pipeline better than few large ones; a second wave costs more than either
+        // (measured at L=48, Ntau=480: 15 -> 51.3, 16 (two waves) -> 55.5, 24 -> 52.4 us per PCG iteration; profiles/).
+        tile = 24;
+        for (int tr = 8; tr <= 32; ++tr) {
+            const long long nct = (long long)gx * ((c->g.Nt + tr - 1) / tr);
+            const size_t per_cta = (size_t)(tr + 2 * W) * 128 * c->esz + 384 + 1024;     // dynamic + static + reserved
+            const long long per_sm = std::min<long long>(16, (long long)(233472 / per_cta));
+            if (nct <= HQMC_MAX_PART && nct <= per_sm * c->n_sm) { tile = tr; break; }
+        }
+    }
     if (tile > c->g.Nt) tile = c->g.Nt;
     if (c->pc_kind == 2 && tile > 96) tile = 96;                 // tile rows (tile + 2W <= 108) x 128 sites x 16 B <= 216 KB
     while ((long long)gx * ((c->g.Nt + tile - 1) / tile) > HQMC_MAX_PART) ++tile;

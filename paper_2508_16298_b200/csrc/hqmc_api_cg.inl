@@ -19,20 +19,34 @@ template <typename T> static int cg_iteration(hqmc_ctx *c, void *x, int par) {
                       (const double *)c->d_part_rz[par], (const double *)c->d_part_rz[par ^ 1], c->n_part_f,
                       (const double *)c->d_part_dOd, c->grid_mdagm, (const double *)c->d_part_rr, c->d_state);
     }
+    // O d is dead once r has been updated, so z = P r is written over it: the iteration's live set is x, r, d, (Od|z) and
+    // the packed phases, 88 MB at config 4, and stays largely L2-resident.
+    void *zb = c->d_Od;
+    if (c->cg_defer_x) {       // x += alpha d rides on the d update: d is streamed once per iteration
+        c->pdl_next = true;
+        HQ_TRY(launch(c, HQMC_K_AXPY, k_cg_raxpy<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_r, (const T2 *)c->d_Od,
+                      (const double *)c->d_part_rz[par], c->n_part_rz, (const double *)c->d_part_dOd, c->grid_mdagm, c->d_part_rr,
+                      c->d_state));
+        HQ_TRY(do_precond<T>(c, c->d_r, zb, c->d_part_rz[par ^ 1], 2));
+        c->pdl_next = true;
+        return launch(c, HQMC_K_DUPDATE, k_cg_xdupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_d,
+                      (const T2 *)zb, (const double *)c->d_part_rz[par ^ 1], (const double *)c->d_part_rz[par], c->n_part_rz,
+                      (const double *)c->d_part_dOd, c->grid_mdagm, (const CgState *)c->d_state);
+    }
     c->pdl_next = true;
     HQ_TRY(launch(c, HQMC_K_AXPY, k_cg_axpy<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_r, (const T2 *)c->d_d,
                   (const T2 *)c->d_Od, (const double *)c->d_part_rz[par], c->n_part_rz, (const double *)c->d_part_dOd,
                   c->grid_mdagm, c->d_part_rr, (const CgState *)c->d_state));
-    HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[par ^ 1], 2));
+    HQ_TRY(do_precond<T>(c, c->d_r, zb, c->d_part_rz[par ^ 1], 2));
     c->pdl_next = true;
-    HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)c->d_z,
+    HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)zb,
                   (const double *)c->d_part_rz[par ^ 1], (const double *)c->d_part_rz[par], c->n_part_rz, 0,
                   (const CgState *)c->d_state));
     return HQMC_OK;
 }
 
 template <typename T> static int cg_build_graph(hqmc_ctx *c, void *x) {
-    if (c->cg_graph && c->cg_graph_x == x && c->cg_graph_tile == c->time_tile && c->cg_graph_fused == c->cg_fused) return HQMC_OK;
+    if (c->cg_graph && c->cg_graph_x == x && c->cg_graph_tile == c->time_tile && c->cg_graph_fused == c->cg_fused && c->cg_graph_defer == c->cg_defer_x) return HQMC_OK;
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     for (int i = 0; i < HQMC_K_COUNT; ++i) c->graph_nodes[i] = 0;
     cudaGraph_t graph = nullptr;
@@ -50,6 +64,7 @@ template <typename T> static int cg_build_graph(hqmc_ctx *c, void *x) {
     c->cg_graph_x = x;
     c->cg_graph_tile = c->time_tile;
     c->cg_graph_fused = c->cg_fused;
+    c->cg_graph_defer = c->cg_defer_x;
     return HQMC_OK;
 }
 

@@ -64,7 +64,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     c->esz = (prm->prec == HQMC_C128) ? 16 : 8;
     c->own_stream = (cuda_stream == nullptr);
     c->stream = (cudaStream_t)cuda_stream;
-    c->cg_graph = nullptr; c->cg_graph_x = nullptr; c->cg_graph_tile = 0; c->cg_graph_fused = false; c->cg_chunk = 32;
+    c->cg_graph = nullptr; c->cg_graph_x = nullptr; c->cg_graph_tile = 0; c->cg_graph_fused = false; c->cg_graph_defer = false; c->cg_defer_x = false; c->cg_chunk = 32;
     c->profiling = false; c->capturing = false; c->theta_set = false; c->skip_mask = 0; c->cg_fused = false; c->pdl = false; c->pdl_next = false;
     c->fused_allowed = false;   // fused PCG vector kernels measured no faster at L=48: opt-in
     for (int i = 0; i < HQMC_K_COUNT; ++i) { c->launches[i] = 0; c->graph_nodes[i] = 0; c->ms[i] = 0.0; }
@@ -275,8 +275,9 @@ extern "C" int hqmc_set_pdl(hqmc_ctx *c, int on) {
     return HQMC_OK;
 }
 extern "C" int hqmc_set_cg_fusion(hqmc_ctx *c, int on) {
-    if (!c) return HQMC_EINVAL;
-    c->fused_allowed = on != 0;
+    if (!c || on < 0 || on > 2) return HQMC_EINVAL;
+    c->cg_defer_x = (on == 2);                        // 2: iterate update deferred into the d update
+    c->fused_allowed = on == 1;
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     precond_cfg(c, c->pc_kind == 1 ? -c->pc_tile : c->pc_tile);
     return HQMC_OK;

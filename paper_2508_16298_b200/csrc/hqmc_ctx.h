@@ -92,7 +92,8 @@ struct hqmc_ctx {
     cudaGraphExec_t cg_graph;
     void *cg_graph_x;        // x pointer baked into the graph
     int cg_graph_tile;
-    bool cg_graph_fused;
+    bool cg_graph_fused, cg_graph_defer;
+    bool cg_defer_x;     // deferred-x PCG vector kernels (k_cg_raxpy + k_cg_xdupdate)
     int cg_chunk;            // iterations per graph launch
     // instrumentation
     bool pdl_next;        // set by a call site whose kernel calls griddepcontrol.wait; consumed by launch()

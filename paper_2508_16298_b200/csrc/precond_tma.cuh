@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(128) k_precond_tma(Geo g, Taps taps, const typ
         if (threadIdx.x == 0) {
             if (mode == 1) {
                 st->bb = rr; st->rr = rr; st->iters = 0;
-                st->done = (rr == 0.0 || st->max_iter <= 0) ? 1 : 0;
+                st->done = (rr == 0.0 || st->max_iter <= 0) ? 2 : 0;     // 2: finished, no iterate update pending
             } else {
                 long long it = st->iters + 1;
                 st->iters = it; st->rr = rr;

@@ -126,7 +126,7 @@ class HQMC:
     def set_precond_tile(self, slices_per_run: int):
         _check(_lib.hqmc_set_precond_tile(self._ctx, C.c_int(slices_per_run)))
 
-    def set_cg_fusion(self, on: bool):
+    def set_cg_fusion(self, on: int):
         _check(_lib.hqmc_set_cg_fusion(self._ctx, C.c_int(int(on))))
 
     def set_pdl(self, on: bool):
