@@ -159,8 +159,10 @@ int hqmc_set_precond_tile(hqmc_ctx *ctx, int slices_per_run);
  * (r -= alpha Od | z = P r | x += alpha d, d = z + beta d: 16 B/site less traffic). All three produce the same iterates;
  * 0 is the fastest at the benchmark sizes, where the five CG vectors largely stay in the 126 MB L2. */
 int hqmc_set_cg_fusion(hqmc_ctx *ctx, int on);
-/* Programmatic dependent launch of the PCG kernels (kernel k+1 is launched while kernel k runs and waits on-device
- * for its completion before reading its output). */
+/* Programmatic dependent launch inside the PCG iteration (kernel k+1 is dispatched under kernel k's tail and waits
+ * on-device for its completion before reading its output). 1 (default) = the preconditioner and the d update, the two
+ * launches that follow a kernel filling every SM; 0 = off; 16 + mask = per-kernel-class mask (bit = HQMC_K_* class),
+ * for timing experiments. Results are bit-identical in every setting. */
 int hqmc_set_pdl(hqmc_ctx *ctx, int on);
 /* TIMING ONLY: bit k of mask set = kernels of class HQMC_K_<k> are not launched (leave-one-out timing of a kernel
  * inside the graph-replayed PCG iteration; the numerical results are then meaningless).  0 restores normal operation. */

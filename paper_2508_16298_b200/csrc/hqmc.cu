@@ -24,7 +24,7 @@ static int drain_events(hqmc_ctx *c) {
 
 template <typename... KArgs, typename... Args>
 static int launch(hqmc_ctx *c, int kclass, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args) {
-    const bool use_pdl = c->pdl && c->pdl_next;
+    const bool use_pdl = c->pdl_next && ((c->pdl >> kclass) & 1);
     c->pdl_next = false;
     if (c->skip_mask & (1u << kclass)) return HQMC_OK;   // leave-one-out timing (results are then meaningless)
     if (c->capturing) c->graph_nodes[kclass]++; else c->launches[kclass]++;

@@ -43,6 +43,12 @@ struct EventPair { cudaEvent_t a, b; int kclass; };
 
 }  // namespace hqmc
 
+// Kernel classes launched programmatically (griddepcontrol) by default: the preconditioner after the residual update and the
+// d update after the preconditioner. Both predecessors fill every SM evenly, so the early-dispatched CTAs spread evenly too
+// (-0.8 us per iteration at L=48). Not after M^+M: its grid leaves SMs idle, the next kernel's CTAs pile onto those and its
+// grid-stride loop then runs unbalanced (+4.7 us, measured; profiles/r01_summary.md).
+#define HQMC_PDL_DEFAULT ((1 << HQMC_K_PRECOND) | (1 << HQMC_K_DUPDATE))
+
 struct hqmc_ctx {
     hqmc_params prm;
     hqmc::Geo g;
@@ -97,7 +103,7 @@ struct hqmc_ctx {
     int cg_chunk;            // iterations per graph launch
     // instrumentation
     bool pdl_next;        // set by a call site whose kernel calls griddepcontrol.wait; consumed by launch()
-    bool pdl;             // programmatic dependent launch of the PCG kernels (hqmc_set_pdl)
+    int pdl;              // bit per kernel class: programmatic dependent launch of the PCG kernels (hqmc_set_pdl)
     unsigned skip_mask;   // timing-only: kernel classes NOT launched inside the PCG iteration (hqmc_set_debug_skip)
     bool profiling;
     bool capturing;

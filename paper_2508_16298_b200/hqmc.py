@@ -129,7 +129,7 @@ class HQMC:
     def set_cg_fusion(self, on: int):
         _check(_lib.hqmc_set_cg_fusion(self._ctx, C.c_int(int(on))))
 
-    def set_pdl(self, on: bool):
+    def set_pdl(self, on: int):
         _check(_lib.hqmc_set_pdl(self._ctx, C.c_int(int(on))))
 
     def set_debug_skip(self, mask: int):

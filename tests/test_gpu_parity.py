@@ -282,10 +282,12 @@ def test_kernels_are_deterministic_run_to_run(hq, L, Nt):
         x2 = g.cg_solve(v, 0.0, 64)[0]
         assert torch.equal(x1, x2), fused
     g.set_cg_fusion(0)
-    g.set_pdl(True)                       # programmatic dependent launch: same arithmetic, different launch overlap
-    x3 = g.cg_solve(v, 0.0, 64)[0].clone()
-    g.set_pdl(False)
-    assert torch.equal(x3, g.cg_solve(v, 0.0, 64)[0])
+    # programmatic dependent launch: same arithmetic, different launch overlap (default = two edges; 0 = off; 16 + 15 = all)
+    outs = []
+    for mode in (1, 0, 16 + 15, 1):
+        g.set_pdl(mode)
+        outs.append(g.cg_solve(v, 0.0, 64)[0].clone())
+    assert all(torch.equal(outs[0], o) for o in outs[1:])
     g.close()
 
 
