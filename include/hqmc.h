@@ -153,11 +153,11 @@ int hqmc_set_mdagm_kernel(hqmc_ctx *ctx, int which);
 /* Preconditioner kernel for W = 1..6: n > 0: TMA-tiled kernel, runs of n slices per CTA; n < 0: register-ring
  * kernel with runs of -n slices; 0 = library default (TMA-tiled). */
 int hqmc_set_precond_tile(hqmc_ctx *ctx, int slices_per_run);
-/* PCG vector kernels: 0 (default) = the textbook four kernels per iteration (M^+M | x += alpha d, r -= alpha Od |
- * z = P r | d = z + beta d); 1 = fused residual-update + preconditioner and fused x/d update where the TMA-tiled
- * preconditioner applies (3 kernels per iteration); 2 = four kernels with the iterate update deferred into the d update
- * (r -= alpha Od | z = P r | x += alpha d, d = z + beta d: 16 B/site less traffic). All three produce the same iterates;
- * 0 is the fastest at the benchmark sizes, where the five CG vectors largely stay in the 126 MB L2. */
+/* PCG vector kernels. 0 (default) = chosen by footprint: the textbook four kernels per iteration (M^+M | x += alpha d,
+ * r -= alpha Od | z = P r | d = z + beta d) while the loop's live set (r, d, Od|z, packed phases) fits the L2, the deferred-x
+ * four otherwise; 1 = fused residual-update + preconditioner and fused x/d update where the TMA-tiled preconditioner
+ * applies (3 kernels per iteration); 2 = deferred-x forced (r -= alpha Od | z = P r | x += alpha d, d = z + beta d:
+ * 16 B/site less traffic); 3 = textbook forced. All produce the same iterates. */
 int hqmc_set_cg_fusion(hqmc_ctx *ctx, int on);
 /* Programmatic dependent launch inside the PCG iteration (kernel k+1 is dispatched under kernel k's tail and waits
  * on-device for its completion before reading its output). 1 (default) = the preconditioner and the d update, the two

@@ -78,6 +78,8 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     cudaDeviceProp prop;
     { cudaError_t e = cudaGetDeviceProperties(&prop, dev); if (e != cudaSuccess) { g_last_error = cudaGetErrorString(e); return fail(HQMC_ECUDA); } }
     c->n_sm = prop.multiProcessorCount;
+    c->l2_bytes = (size_t)prop.l2CacheSize;
+    c->cg_defer_x = cg_defer_default(c);
     if (nb <= 256) c->cfg = {1, 256, 0};
     else if (nb <= 576) c->cfg = {1, 576, 0};
     else if (nb <= 1152) c->cfg = {2, 576, 0};
@@ -275,8 +277,8 @@ extern "C" int hqmc_set_pdl(hqmc_ctx *c, int on) {
     return HQMC_OK;
 }
 extern "C" int hqmc_set_cg_fusion(hqmc_ctx *c, int on) {
-    if (!c || on < 0 || on > 2) return HQMC_EINVAL;
-    c->cg_defer_x = (on == 2);                        // 2: iterate update deferred into the d update
+    if (!c || on < 0 || on > 3) return HQMC_EINVAL;
+    c->cg_defer_x = on == 2 || (on == 0 && cg_defer_default(c));
     c->fused_allowed = on == 1;
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     precond_cfg(c, c->pc_kind == 1 ? -c->pc_tile : c->pc_tile);

@@ -99,6 +99,7 @@ struct hqmc_ctx {
     void *cg_graph_x;        // x pointer baked into the graph
     int cg_graph_tile;
     bool cg_graph_fused, cg_graph_defer;
+    size_t l2_bytes;     // device L2 size
     bool cg_defer_x;     // deferred-x PCG vector kernels (k_cg_raxpy + k_cg_xdupdate)
     int cg_chunk;            // iterations per graph launch
     // instrumentation
@@ -113,3 +114,9 @@ struct hqmc_ctx {
     std::vector<hqmc::EventPair> pending;
     std::vector<hqmc::EventPair> pool;
 };
+
+// The PCG loop's live set is r, d, Od|z and the packed phases (4 x N x esz; x is streamed). While it fits the L2 the textbook
+// kernels win (their traffic is L2 traffic); beyond it the deferred-x pair, which moves 16 B/site less, does
+// (L=64, Ntau=640, 168 MB: 128.9 vs 131.5 us per iteration; L=48, Ntau=480, 71 MB: 53.2 vs 52.4; profiles/r01_summary.md).
+static bool cg_defer_default(const hqmc_ctx *c) { return 4 * c->N * c->esz > c->l2_bytes; }
+

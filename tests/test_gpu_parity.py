@@ -120,13 +120,13 @@ def test_cg_solution_and_iterations(hq, L, Nt, seed, W):
 
 @pytest.mark.parametrize("L,Nt,seed,W", [(8, 40, 2, 6), (12, 30, 3, 3), (6, 10, 1, 1)])
 def test_cg_fused_and_unfused_kernels_agree_with_oracle(hq, L, Nt, seed, W):
-    """Textbook 4-kernel (0, default), fused 3-kernel (1) and deferred-x (2) iterations all give the oracle's iterates."""
+    """Default (0), fused 3-kernel (1), deferred-x (2) and textbook 4-kernel (3) iterations all give the oracle's iterates."""
     o, g, theta = setup(hq, L, Nt, seed, W=W)
     eta = inputs.complex_gaussian((Nt, L, L), seed)
     phi = o.apply_Mdag(theta, eta)
     xo, ito, relo = o.pcg(theta, phi, 0.0, 25)
     x_ref, it_ref, _ = o.pcg(theta, phi, 1e-10, 100000)
-    for fused in (1, 0, 2):
+    for fused in (1, 0, 2, 3):
         g.set_cg_fusion(fused)
         for tile in (0, 7):
             g.set_precond_tile(tile)
@@ -276,7 +276,7 @@ def test_kernels_are_deterministic_run_to_run(hq, L, Nt):
         g.set_mdagm_kernel(0)
     except hq.HqmcError:
         g.set_mdagm_kernel(3)
-    for fused in (0, 1, 2):
+    for fused in (0, 1, 2, 3):
         g.set_cg_fusion(fused)
         x1 = g.cg_solve(v, 0.0, 64)[0].clone()
         x2 = g.cg_solve(v, 0.0, 64)[0]
