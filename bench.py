@@ -373,6 +373,41 @@ def run_solve(args):
     return 0
 
 
+def run_measure(args):
+    """--mode measure: the stochastic estimator (widening row NEXT-2) on a paper-regime field of the chosen
+    config: n_rv noise vectors -> G xi by PCG -> the pair correlator over binom(n_rv, 2) pairs through Eq.19 (cuFFT).  Not the
+    timed metric; reports time per stage."""
+    import torch
+    from paper_2508_16298_b200 import hqmc, inputs
+    c = inputs.CONFIGS[args.config]
+    L, Ntau, n_rv = c["L"], c["Ntau"], args.n_rv
+    theta = inputs.theta_paper_regime(L, Ntau, c["seed"])
+    g = hqmc.HQMC(L, Ntau)
+    g.set_theta(torch.from_numpy(theta).cuda())
+    xi = torch.from_numpy(np.stack([inputs.complex_gaussian((Ntau, L, L), c["seed"] + 10 * k, inputs.STREAM_VEC) for k in range(n_rv)])).cuda()
+    gv = torch.empty_like(xi)
+    out = g.new_vec()
+
+    def timed(fn):
+        fn(); torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); r = fn(); e1.record(); torch.cuda.synchronize()
+        return r, e0.elapsed_time(e1)
+
+    (_, iters, ok), ms_solve = timed(lambda: g.green_apply(xi, args.tol, args.max_iter, out=gv))
+    _, ms_2pt = timed(lambda: g.green_2pt(gv, xi, out=out))
+    _, ms_pair = timed(lambda: g.pair_correlator(gv, xi, out=out))
+    back = g.apply_M(gv[0].contiguous())
+    res = float(torch.linalg.vector_norm(back - xi[0]) / torch.linalg.vector_norm(xi[0]))
+    npair = n_rv * (n_rv - 1) // 2
+    print(json.dumps({"mode": "measure", "config": args.config, "L": L, "Ntau": Ntau, "n_rv": n_rv, "tol": args.tol,
+                      "theta": "paper regime (c_tau=80, K=1 heat bath, cold start)", "converged": ok, "cg_iters_total": iters,
+                      "ms_green_apply": ms_solve, "ms_per_vector": ms_solve / n_rv, "relres_M_Gxi_minus_xi": res,
+                      "ms_green_2pt": ms_2pt, "pairs": npair, "ms_pair_correlator": ms_pair, "us_per_pair": 1e3 * ms_pair / npair}))
+    g.close()
+    return 0
+
+
 def mdagm_sweep(g, torch, dev, L, Ntau, prec, nbuf=8, reps=25):
     """M^+M alone: cold = rotate nbuf distinct (in, out) pairs so every launch streams from HBM; warm = one pair."""
     N = L * L * Ntau
@@ -412,7 +447,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--prec", default="c128", choices=["c128", "c64"])
     ap.add_argument("--no-sweep", action="store_true")
-    ap.add_argument("--mode", default="step", choices=["step", "solve"], help="solve: one full PCG solve to --tol (not the timed metric)")
+    ap.add_argument("--mode", default="step", choices=["step", "solve", "measure"],
+                    help="solve: one full PCG solve to --tol; measure: the stochastic estimator on a paper-regime field (neither is the timed metric)")
+    ap.add_argument("--n-rv", type=int, default=40, help="measure mode: number of noise vectors (PAPER.md:244)")
     ap.add_argument("--tol", type=float, default=1e-10)
     ap.add_argument("--theta", default="config", choices=["config", "paper"], help="solve mode: the config's field or a paper-regime field")
     ap.add_argument("--max-iter", type=int, default=3000000)
@@ -421,6 +458,8 @@ def main():
         args.warmup = 3
     if args.mode == "solve":
         return run_solve(args)
+    if args.mode == "measure":
+        return run_measure(args)
     return run_reference(args) if args.impl == "reference" else run_gpu(args)
 
 

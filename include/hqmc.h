@@ -120,6 +120,30 @@ int hqmc_hqmc_step(hqmc_ctx *ctx, double *d_theta, double *d_p, const void *d_et
                    double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out, int *accepted_out,
                    long long *cg_iters_out);
 
+/* ---- Stochastic estimation of fermionic observables ----
+ * All pointers are DEVICE pointers to lattice vectors [Ntau][L][L] of the context's complex type (n_rv of them back to
+ * back where a count is given), 16-byte aligned, caller-owned.  The calls enqueue on the context's stream; cuFFT provides
+ * the transforms of Eq.19 (plan created on first use and owned by the context). */
+
+/* g_k = G xi_k = (M^+ M)^{-1} R_k,  R_k := M^+ xi_k, k = 0..n_rv-1, each by the PCG of Eq.20 to the
+ * relative residual `tol` (at most max_iter iterations per vector).  *iters_total (host, may be NULL): iterations summed
+ * over the vectors.  Needs hqmc_set_theta.  d_xi and d_g must not overlap.  Returns HQMC_ENOCONV if any solve did not
+ * reach tol (all results are still written). */
+int hqmc_green_apply(hqmc_ctx *ctx, const void *d_xi, void *d_g, int n_rv, double tol, long long max_iter,
+                     long long *iters_total);
+
+/* Eq.17-19: C(Delta) = (1/N) sum_i a_i b_{i+Delta} = (1/N) F^{-1}[F[a]_{-k} F[b]_k](Delta), i + Delta periodic in tau, y and
+ * x (reading C23), N = L*L*Ntau.  d_C may alias d_a or d_b. */
+int hqmc_translation_average(hqmc_ctx *ctx, const void *d_a, const void *d_b, void *d_C);
+
+/* Translation average of the two-point estimate G^_ij = [G xi]_i xi_j^* (PAPER.md:240): a = g_k, b = conj(xi_k), mean over
+ * the n_rv vectors (accumulated in Fourier space, one inverse transform). */
+int hqmc_green_2pt(hqmc_ctx *ctx, const void *d_g, const void *d_xi, int n_rv, void *d_C);
+
+/* The paper's example C(i,j) = G_ij G_ij: a_i = (G xi)_i (G xi')_i, b_j = xi_j^* xi'_j^*, Eq.19 for
+ * every unordered pair of the n_rv >= 2 vectors, mean over the binom(n_rv, 2) pairs. */
+int hqmc_pair_correlator(hqmc_ctx *ctx, const void *d_g, const void *d_xi, int n_rv, void *d_C);
+
 /* HOST-buffer variants (pageable or pinned host memory; the copies run inside the call on the
  * context's stream and the call returns after the result has landed in h_out / h_x). */
 int hqmc_apply_MdagM_host(hqmc_ctx *ctx, const void *h_in, void *h_out);

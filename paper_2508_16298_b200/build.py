@@ -9,10 +9,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhqmc.so")
 SOURCES = ["hqmc.cu"]
-DEPS = ["block_engine.cuh", "kernels.cuh", "mdagm_stream.cuh", "tma.cuh", "mdagm_ws.cuh", "mdagm_cluster.cuh", "mdagm_back.cuh", "precond_tma.cuh", "cg_kernels.cuh", "force_kernels.cuh", "hqmc_ctx.h", "hqmc_api_setup.inl",
-        "hqmc_api_cg.inl", "hqmc_api_md.inl", os.path.join("..", "..", "include", "hqmc.h")]
+DEPS = ["block_engine.cuh", "kernels.cuh", "mdagm_stream.cuh", "tma.cuh", "mdagm_ws.cuh", "mdagm_cluster.cuh", "mdagm_back.cuh", "precond_tma.cuh", "measure_kernels.cuh", "cg_kernels.cuh", "force_kernels.cuh", "hqmc_ctx.h", "hqmc_api_setup.inl",
+        "hqmc_api_cg.inl", "hqmc_api_md.inl", "hqmc_api_measure.inl", os.path.join("..", "..", "include", "hqmc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
-              "-shared", "--expt-relaxed-constexpr", "-cudart", "static"]
+              "-shared", "--expt-relaxed-constexpr", "-cudart", "static",
+              "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]      # cuFFT: the FFT of Eq.19 (library primitive)
 
 
 def needs_build() -> bool:

@@ -340,3 +340,4 @@ using namespace hqmc;
 #include "hqmc_api_setup.inl"
 #include "hqmc_api_cg.inl"
 #include "hqmc_api_md.inl"
+#include "hqmc_api_measure.inl"

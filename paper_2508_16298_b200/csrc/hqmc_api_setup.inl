@@ -169,7 +169,8 @@ extern "C" int hqmc_destroy(hqmc_ctx *c) {
     if (c->cg_graph) cudaGraphExecDestroy(c->cg_graph);
     for (auto &ep : c->pending) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (auto &ep : c->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-    void *ptrs[] = {c->d_halo, c->d_flags, c->d_r2, c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
+    if (c->ms_plan_ok) cufftDestroy(c->ms_plan);
+    void *ptrs[] = {c->d_ms_a, c->d_ms_b, c->d_ms_acc, c->d_halo, c->d_flags, c->d_r2, c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
                     c->d_part_rr, c->d_part_rz[0], c->d_part_rz[1], c->d_part_misc, c->d_state, c->d_scal};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (c->h_state) cudaFreeHost(c->h_state);

@@ -1,6 +1,7 @@
 // hqmc_ctx.h -- private context of libhqmc.so and launch helpers (host code).
 #pragma once
 #include <cuda_runtime.h>
+#include <cufft.h>
 
 #include <cmath>
 #include <cstdint>
@@ -18,6 +19,7 @@
 #include "mdagm_cluster.cuh"
 #include "mdagm_back.cuh"
 #include "precond_tma.cuh"
+#include "measure_kernels.cuh"
 
 namespace hqmc {
 
@@ -100,6 +102,10 @@ struct hqmc_ctx {
     int cg_graph_tile;
     bool cg_graph_fused, cg_graph_defer;
     size_t l2_bytes;     // device L2 size
+    // stochastic estimator (hqmc_api_measure.inl): workspace and 3-D FFT plan, created on first use
+    bool ms_ready = false, ms_plan_ok = false;
+    cufftHandle ms_plan = 0;
+    void *d_ms_a = nullptr, *d_ms_b = nullptr, *d_ms_acc = nullptr;
     bool cg_defer_x;     // deferred-x PCG vector kernels (k_cg_raxpy + k_cg_xdupdate)
     int cg_chunk;            // iterations per graph launch
     // instrumentation

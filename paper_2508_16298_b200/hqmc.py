@@ -23,7 +23,8 @@ KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
-    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
+    "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_fusion", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
@@ -197,6 +198,42 @@ class HQMC:
                                        C.c_double(u), C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter),
                                        C.byref(H0), C.byref(H1), C.byref(acc), C.byref(it)), allow_noconv=True)
         return dict(H0=H0.value, H1=H1.value, accepted=bool(acc.value), cg_iters=it.value, converged=(s == HQMC_OK))
+
+    # ---- stochastic estimator -------------------------------------------------
+    def _vecs(self, v):
+        assert v.is_cuda and v.dtype == self.cdtype and v.is_contiguous() and v.numel() % self.N == 0 and v.numel() >= self.N
+        return v, v.numel() // self.N
+
+    def green_apply(self, xi, tol=1e-10, max_iter=1000000, out=None):
+        """g_k = (M^+M)^{-1} M^+ xi_k for the stacked vectors xi [n_rv][Ntau][L][L] -> (g, total iterations, converged)."""
+        xi, n = self._vecs(xi)
+        out = torch.empty_like(xi) if out is None else out
+        it = C.c_longlong(0)
+        s = _check(_lib.hqmc_green_apply(self._ctx, _ptr(xi), _ptr(out), C.c_int(n), C.c_double(tol), C.c_longlong(max_iter),
+                                         C.byref(it)), allow_noconv=True)
+        return out, it.value, s == HQMC_OK
+
+    def translation_average(self, a, b, out=None):
+        """Eq.17-19: C(Delta) = (1/N) sum_i a_i b_{i+Delta}."""
+        out = self.new_vec() if out is None else out
+        _check(_lib.hqmc_translation_average(self._ctx, _ptr(self._vec(a)), _ptr(self._vec(b)), _ptr(self._vec(out))))
+        return out
+
+    def green_2pt(self, g, xi, out=None):
+        g, n = self._vecs(g)
+        xi, n2 = self._vecs(xi)
+        assert n == n2
+        out = self.new_vec() if out is None else out
+        _check(_lib.hqmc_green_2pt(self._ctx, _ptr(g), _ptr(xi), C.c_int(n), _ptr(self._vec(out))))
+        return out
+
+    def pair_correlator(self, g, xi, out=None):
+        g, n = self._vecs(g)
+        xi, n2 = self._vecs(xi)
+        assert n == n2 and n >= 2
+        out = self.new_vec() if out is None else out
+        _check(_lib.hqmc_pair_correlator(self._ctx, _ptr(g), _ptr(xi), C.c_int(n), _ptr(self._vec(out))))
+        return out
 
     # ---- host-buffer entry points (numpy arrays, pageable or pinned) ----------------------------
     def apply_MdagM_host(self, h_in: np.ndarray, h_out: np.ndarray):
