@@ -48,7 +48,8 @@ typedef struct {
     double dtau, t;    /* Trotter step 0.1 and hopping 1                         */
     double c_tau, K;   /* S_B couplings: c_tau = 1/(J dtau^2), K (reading C12)     */
     int compact;       /* 1: compact L_B^c; 0: non-compact L_B^nc (Eq.2) */
-    int precond_W;     /* preconditioner half bandwidth in tau, 0..32; 0 = identity (reading C10)  */
+    int precond_W;     /* preconditioner half bandwidth in tau, 0..32; 0 = identity (reading C10);  */
+                       /* 1..12 run the TMA-tiled kernel, wider ones the generic kernel              */
     hqmc_prec prec;    /* arithmetic of the fermion vectors                                        */
 } hqmc_params;
 

@@ -21,7 +21,7 @@ __global__ void __launch_bounds__(128) k_precond_tma(Geo g, Taps taps, const typ
                                                      typename Cx<T>::type *__restrict__ z, double *__restrict__ part_rz,
                                                      const double *__restrict__ part_rr, int n_rr, CgState *st, int mode, int TR) {
     typedef typename Cx<T>::type T2;
-    static_assert(W >= 1 && W <= 6, "register ring of 13 slots");
+    static_assert(W >= 1 && W <= 12, "register ring of 2W+1 <= 25 slots");
     constexpr int RING = 2 * W + 1;
     pdl_wait();
     if (mode != 0 && *(volatile const int *)&st->done) return;

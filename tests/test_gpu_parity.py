@@ -74,7 +74,8 @@ def test_config2_twenty_MdagM(hq):
     g.close()
 
 
-@pytest.mark.parametrize("L,Nt,W", [(4, 8, 6), (6, 10, 3), (12, 30, 6), (4, 8, 0), (12, 41, 6), (14, 20, 1), (6, 40, 8)])
+@pytest.mark.parametrize("L,Nt,W", [(4, 8, 6), (6, 10, 3), (12, 30, 6), (4, 8, 0), (12, 41, 6), (14, 20, 1), (6, 40, 8), (8, 30, 7), (6, 40, 10),
+                                    (12, 41, 12), (6, 40, 13)])   # 1..6: TMA or register-ring kernel; 7..12: TMA kernel; 13+: generic kernel
 def test_precond_and_taps(hq, L, Nt, W):
     o, g, theta = setup(hq, L, Nt, 3, W=W)
     if W > 0:
@@ -88,7 +89,7 @@ def test_precond_and_taps(hq, L, Nt, W):
     g.close()
 
 
-@pytest.mark.parametrize("L,Nt,seed,W", [(4, 8, 0, 6), (4, 8, 0, 0), (6, 10, 1, 6), (8, 40, 2, 6)])
+@pytest.mark.parametrize("L,Nt,seed,W", [(4, 8, 0, 6), (4, 8, 0, 0), (6, 10, 1, 6), (8, 40, 2, 6), (8, 40, 2, 10)])
 def test_cg_solution_and_iterations(hq, L, Nt, seed, W):
     o, g, theta = setup(hq, L, Nt, seed, W=W)
     eta = inputs.complex_gaussian((Nt, L, L), seed)
