@@ -52,15 +52,15 @@ __global__ void __launch_bounds__(128) k_precond_tma(Geo g, Taps taps, const typ
     }
     __syncthreads();
     // row i of the tile = time ta - W + i, with the antiperiodic sign of the wrap
-    auto ld = [&](int i) -> T2 {
+    // the ring holds doubles whatever T is: a complex64 row is widened once, when it enters the ring
+    auto ld = [&](int i) -> double2 {
         if ((i & (HQMC_PC_ROWS_PER_BAR - 1)) == 0) mbar_wait(&bars[i / HQMC_PC_ROWS_PER_BAR], 0);
         const int u = ta - W + i;
-        const T sg = (u < 0 || u >= Nt) ? (T)-1 : (T)1;
-        T2 v = tile[(size_t)i * 128 + threadIdx.x];
-        v.x *= sg; v.y *= sg;
-        return v;
+        const double sg = (u < 0 || u >= Nt) ? -1.0 : 1.0;
+        const T2 v = tile[(size_t)i * 128 + threadIdx.x];
+        return make_double2(sg * (double)v.x, sg * (double)v.y);
     };
-    T2 ring[RING];
+    double2 ring[RING];
 #pragma unroll
     for (int j = 0; j < 2 * W; ++j) ring[j] = ld(j);       // times ta-W .. ta+W-1
     double acc = 0.0;
@@ -71,18 +71,18 @@ __global__ void __launch_bounds__(128) k_precond_tma(Geo g, Taps taps, const typ
             const int tt = t + j;
             if (tt < tb) {
                 ring[(j + 2 * W) % RING] = ld(tt - ta + 2 * W);            // time tt + W
-                const T2 c = ring[(j + W) % RING];
-                double zx = taps.p[0] * (double)c.x, zy = taps.p[0] * (double)c.y;
+                const double2 c = ring[(j + W) % RING];
+                double zx = taps.p[0] * c.x, zy = taps.p[0] * c.y;
 #pragma unroll
                 for (int m = 1; m <= W; ++m) {
-                    const T2 a = ring[(j + W + m) % RING], b = ring[(j + W - m) % RING];
-                    zx = fma(taps.p[m], (double)a.x + (double)b.x, zx);
-                    zy = fma(taps.p[m], (double)a.y + (double)b.y, zy);
+                    const double2 a = ring[(j + W + m) % RING], b = ring[(j + W - m) % RING];
+                    zx = fma(taps.p[m], a.x + b.x, zx);
+                    zy = fma(taps.p[m], a.y + b.y, zy);
                 }
                 T2 zi; zi.x = (T)zx; zi.y = (T)zy;
                 if (act) {
                     zs[(size_t)tt * Vs] = zi;
-                    acc += (double)c.x * (double)zi.x + (double)c.y * (double)zi.y;
+                    acc += c.x * (double)zi.x + c.y * (double)zi.y;
                 }
             }
         }
