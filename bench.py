@@ -111,7 +111,8 @@ def oracle_step_sample(L, Ntau, seed, cg_iters, nsteps_md=1, threads=None):
     from oracle import oracle as orc
     from paper_2508_16298_b200 import inputs
     orc.build()
-    threads = threads or orc.max_threads()
+    # torchrun exports OMP_NUM_THREADS=1 for its ranks; only one rank ever runs the oracle, so it takes the cores it may use
+    threads = threads or max(orc.max_threads(), len(os.sched_getaffinity(0)))
     orc.set_threads(threads)
     theta = inputs.theta_uniform(L, Ntau, seed)
     eta = inputs.complex_gaussian((Ntau, L, L), seed)
