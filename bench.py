@@ -374,6 +374,53 @@ def run_solve(args):
     return 0
 
 
+def run_trajectory(args):
+    """--mode trajectory: BASELINE config 5's protocol ("5 HMC trajectories of 20 leapfrog steps each, reporting ms per
+    trajectory and HBM fraction") on the chosen config.  The PCG runs the paper's fixed iteration count per solve
+    (--cg-iters): on BASELINE's rough fields a solve to 1e-10 needs 3-6 x 10^5 iterations (`--mode solve`),
+    i.e. half an hour per trajectory, so tolerance-stopped trajectories are timed on the paper-regime field (--theta paper,
+    --tol) instead.  Not the timed metric of the JSON contract."""
+    import torch
+    from paper_2508_16298_b200 import hqmc, inputs
+    c = inputs.CONFIGS[args.config]
+    L, Ntau = c["L"], c["Ntau"]
+    N = L * L * Ntau
+    paper = args.theta == "paper"
+    theta0 = inputs.theta_paper_regime(L, Ntau, c["seed"]) if paper else inputs.make_theta(args.config)
+    kw = dict(c_tau=80.0, K=1.0) if paper else {}
+    g = hqmc.HQMC(L, Ntau, **kw)
+    tol, cap = (args.tol, args.max_iter) if paper else (0.0, args.cg_iters)
+    d_theta0 = torch.from_numpy(theta0).cuda()
+    times, iters, dH = [], [], []
+    for k in range(args.n_traj + 1):                              # first one is warm-up
+        d_theta = d_theta0.clone()
+        d_p = torch.from_numpy(inputs.momenta(L, Ntau, c["seed"] + k)).cuda()
+        g.set_theta(d_theta)
+        d_phi = g.apply_Mdag(torch.from_numpy(inputs.complex_gaussian((Ntau, L, L), c["seed"] + k)).cuda())
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        r = g.trajectory(d_theta, d_p, d_phi, args.md_steps, args.eps, cg_tol=tol, cg_max_iter=cap)
+        e1.record(); torch.cuda.synchronize()
+        if k:
+            times.append(e0.elapsed_time(e1)); iters.append(r["cg_iters"]); dH.append(r["H1"] - r["H0"])
+    ms = float(np.mean(times))
+    it = float(np.mean(iters))
+    peak, peak_src = measured_peaks()
+    bps = 224.0                                                   # algorithmic bytes per site per PCG iteration (DESIGN.md section 6)
+    print(json.dumps({"mode": "trajectory", "config": args.config, "L": L, "Ntau": Ntau, "sites": N,
+                      "theta": "paper regime (c_tau=80, K=1 heat bath, cold start)" if paper else c["theta"],
+                      "md_steps": args.md_steps, "eps": args.eps, "trajectories": args.n_traj,
+                      "cg": f"to {tol:g}" if paper else f"fixed {cap} iterations per solve (PAPER.md:348)",
+                      "ms_per_trajectory": ms, "ms_min": float(np.min(times)), "ms_max": float(np.max(times)),
+                      "cg_iters_per_trajectory": it, "us_per_cg_iter_all_in": 1e3 * ms / it,
+                      "MdagM_Gsite_per_s": it * N / (ms * 1e-3) / 1e9,
+                      "hbm_fraction_alg": bps * N * it / (ms * 1e-3) / 1e9 / peak, "peak_GBps": peak, "peak_source": peak_src,
+                      "dH": dH}))
+    g.close()
+    return 0
+
+
 def run_measure(args):
     """--mode measure: the stochastic estimator (widening row NEXT-2) on a paper-regime field of the chosen
     config: n_rv noise vectors -> G xi by PCG -> the pair correlator over binom(n_rv, 2) pairs through Eq.19 (cuFFT).  Not the
@@ -448,11 +495,14 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--prec", default="c128", choices=["c128", "c64"])
     ap.add_argument("--no-sweep", action="store_true")
-    ap.add_argument("--mode", default="step", choices=["step", "solve", "measure"],
+    ap.add_argument("--mode", default="step", choices=["step", "solve", "measure", "trajectory"],
                     help="solve: one full PCG solve to --tol; measure: the stochastic estimator on a paper-regime field (neither is the timed metric)")
+    ap.add_argument("--n-traj", type=int, default=5, help="trajectory mode: timed trajectories (BASELINE config 5: 5)")
+    ap.add_argument("--md-steps", type=int, default=20, help="trajectory mode: leapfrog steps per trajectory (BASELINE config 5: 20)")
+    ap.add_argument("--eps", type=float, default=0.05, help="trajectory mode: leapfrog step size")
     ap.add_argument("--n-rv", type=int, default=40, help="measure mode: number of noise vectors (PAPER.md:244)")
     ap.add_argument("--tol", type=float, default=1e-10)
-    ap.add_argument("--theta", default="config", choices=["config", "paper"], help="solve mode: the config's field or a paper-regime field")
+    ap.add_argument("--theta", default="config", choices=["config", "paper"], help="solve / trajectory modes: the config's field or a paper-regime field")
     ap.add_argument("--max-iter", type=int, default=3000000)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
@@ -461,6 +511,8 @@ def main():
         return run_solve(args)
     if args.mode == "measure":
         return run_measure(args)
+    if args.mode == "trajectory":
+        return run_trajectory(args)
     return run_reference(args) if args.impl == "reference" else run_gpu(args)
 
 
