@@ -429,6 +429,8 @@ def run_measure(args):
     from paper_2508_16298_b200 import hqmc, inputs
     c = inputs.CONFIGS[args.config]
     L, Ntau, n_rv = c["L"], c["Ntau"], args.n_rv
+    if args.L:                                               # the paper's shape at another size: V_s = L^2, N_tau = 10 L
+        L, Ntau = args.L, 10 * args.L
     theta = inputs.theta_paper_regime(L, Ntau, c["seed"])
     g = hqmc.HQMC(L, Ntau)
     g.set_theta(torch.from_numpy(theta).cuda())
@@ -442,7 +444,12 @@ def run_measure(args):
         e0.record(); r = fn(); e1.record(); torch.cuda.synchronize()
         return r, e0.elapsed_time(e1)
 
-    (_, iters, ok), ms_solve = timed(lambda: g.green_apply(xi, args.tol, args.max_iter, out=gv))
+    # vectors per launch of the multi-right-hand-side PCG: 0 = library default (by L2 footprint), 1 = one at a time
+    by_batch = {}
+    for bs in [int(b) for b in args.green_batch.split(",")][::-1]:
+        g.set_green_batch(bs)
+        (_, iters, ok), ms_solve = timed(lambda: g.green_apply(xi, args.tol, args.max_iter, out=gv))
+        by_batch[str(bs)] = {"ms_green_apply": ms_solve, "cg_iters_total": iters, "converged": ok}
     _, ms_2pt = timed(lambda: g.green_2pt(gv, xi, out=out))
     _, ms_pair = timed(lambda: g.pair_correlator(gv, xi, out=out))
     back = g.apply_M(gv[0].contiguous())
@@ -450,7 +457,7 @@ def run_measure(args):
     npair = n_rv * (n_rv - 1) // 2
     print(json.dumps({"mode": "measure", "config": args.config, "L": L, "Ntau": Ntau, "n_rv": n_rv, "tol": args.tol,
                       "theta": "paper regime (c_tau=80, K=1 heat bath, cold start)", "converged": ok, "cg_iters_total": iters,
-                      "ms_green_apply": ms_solve, "ms_per_vector": ms_solve / n_rv, "relres_M_Gxi_minus_xi": res,
+                      "green_batch": int(args.green_batch.split(",")[0]), "ms_green_apply": ms_solve, "ms_per_vector": ms_solve / n_rv, "by_green_batch": by_batch, "relres_M_Gxi_minus_xi": res,
                       "ms_green_2pt": ms_2pt, "pairs": npair, "ms_pair_correlator": ms_pair, "us_per_pair": 1e3 * ms_pair / npair}))
     g.close()
     return 0
@@ -501,6 +508,9 @@ def main():
     ap.add_argument("--md-steps", type=int, default=20, help="trajectory mode: leapfrog steps per trajectory (BASELINE config 5: 20)")
     ap.add_argument("--eps", type=float, default=0.05, help="trajectory mode: leapfrog step size")
     ap.add_argument("--n-rv", type=int, default=40, help="measure mode: number of noise vectors (PAPER.md:244)")
+    ap.add_argument("--green-batch", default="0", help="measure mode: vectors per launch of the batched PCG, comma list to compare "
+                    "(0 = library default, 1 = one at a time); the first entry is the one the other stages run after")
+    ap.add_argument("--L", type=int, default=0, help="measure mode: lattice size override (N_tau = 10 L)")
     ap.add_argument("--tol", type=float, default=1e-10)
     ap.add_argument("--theta", default="config", choices=["config", "paper"], help="solve / trajectory modes: the config's field or a paper-regime field")
     ap.add_argument("--max-iter", type=int, default=3000000)

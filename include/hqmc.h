@@ -133,6 +133,18 @@ int hqmc_hqmc_step(hqmc_ctx *ctx, double *d_theta, double *d_p, const void *d_et
 int hqmc_green_apply(hqmc_ctx *ctx, const void *d_xi, void *d_g, int n_rv, double tol, long long max_iter,
                      long long *iters_total);
 
+/* The same PCG for n_vec right-hand sides at once (the N_rv noise vectors share one theta): d_rhs and d_x
+ * hold n_vec lattice vectors back to back (device, 16-byte aligned, caller-owned, must not overlap); vector b is solved
+ * exactly as hqmc_cg_solve would (x_0 = 0, Eq.20, readings C8-C9), with its own alpha, beta and stopping test; one kernel
+ * launch carries all vectors (vector index in the grid), the workspace (4 n_vec vectors) is library-owned and grown on
+ * demand.  iters_out / relres_out: HOST arrays of n_vec entries (may be NULL).  Supported where one thread holds a 2x2
+ * block (L <= 48) and Ntau <= 4096, else HQMC_EINVAL.  Synchronises the stream.  HQMC_ENOCONV if any vector missed tol. */
+int hqmc_cg_solve_batched(hqmc_ctx *ctx, const void *d_rhs, void *d_x, int n_vec, double tol, long long max_iter,
+                          long long *iters_out, double *relres_out);
+/* Vectors hqmc_green_apply solves per launch: 0 (default) = as many as keep the batch's live set L2-resident, 1 = one at a
+ * time on the one-vector kernels, n > 1 = n at a time. */
+int hqmc_set_green_batch(hqmc_ctx *ctx, int n);
+
 /* Eq.17-19: C(Delta) = (1/N) sum_i a_i b_{i+Delta} = (1/N) F^{-1}[F[a]_{-k} F[b]_k](Delta), i + Delta periodic in tau, y and
  * x (reading C23), N = L*L*Ntau.  d_C may alias d_a or d_b. */
 int hqmc_translation_average(hqmc_ctx *ctx, const void *d_a, const void *d_b, void *d_C);

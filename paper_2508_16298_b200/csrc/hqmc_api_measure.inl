@@ -79,6 +79,21 @@ extern "C" int hqmc_green_apply(hqmc_ctx *c, const void *d_xi, void *d_g, int n_
     if (!c || !c->theta_set || !d_xi || !d_g || d_xi == d_g || n_rv < 1 || max_iter < 0 || !aligned16(d_xi) || !aligned16(d_g)) return HQMC_EINVAL;
     long long total = 0;
     int worst = HQMC_OK;
+    const int bs = green_batch_size(c, n_rv);
+    if (bs > 1) {                                  // several vectors per launch (hqmc_api_cgb.inl)
+        std::vector<long long> its((size_t)bs);
+        for (int k = 0; k < n_rv; k += bs) {
+            const int n = std::min(bs, n_rv - k);
+            const char *xi = (const char *)d_xi + (size_t)k * c->N * c->esz;
+            char *g = (char *)d_g + (size_t)k * c->N * c->esz;
+            const int st = DISPATCH_T(c, green_batch_t<double>(c, xi, g, n, tol, max_iter, its.data()),
+                                      green_batch_t<float>(c, xi, g, n, tol, max_iter, its.data()));
+            for (int b = 0; b < n; ++b) total += its[b];
+            if (st == HQMC_ENOCONV) worst = st; else if (st != HQMC_OK) return st;
+        }
+        if (iters_total) *iters_total = total;
+        return worst;
+    }
     for (int k = 0; k < n_rv; ++k) {
         const char *xi = (const char *)d_xi + (size_t)k * c->N * c->esz;
         char *g = (char *)d_g + (size_t)k * c->N * c->esz;

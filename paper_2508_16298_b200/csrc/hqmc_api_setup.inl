@@ -167,6 +167,9 @@ extern "C" int hqmc_destroy(hqmc_ctx *c) {
     if (!c) return HQMC_EINVAL;
     if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
     if (c->cg_graph) cudaGraphExecDestroy(c->cg_graph);
+    if (c->cgb_graph) cudaGraphExecDestroy(c->cgb_graph);
+    { void *bp[] = {c->d_cgb_r, c->d_cgb_d, c->d_cgb_Od, c->d_cgb_phi, c->d_cgb_part, c->d_cgb_state}; for (void *p : bp) if (p) cudaFree(p); }
+    if (c->h_cgb_state) cudaFreeHost(c->h_cgb_state);
     for (auto &ep : c->pending) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (auto &ep : c->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     if (c->ms_plan_ok) cufftDestroy(c->ms_plan);
@@ -187,6 +190,7 @@ extern "C" int hqmc_set_precond(hqmc_ctx *c, int W, const double *taps_host) {
     if (W == 0) c->taps.p[0] = taps_host ? taps_host[0] : 1.0;
     else for (int i = 0; i <= W; ++i) c->taps.p[i] = taps_host[i];
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }   // taps are baked into the graph
+    if (c->cgb_graph) { cudaGraphExecDestroy(c->cgb_graph); c->cgb_graph = nullptr; }
     precond_cfg(c, 0);
     return HQMC_OK;
 }

@@ -20,6 +20,7 @@
 #include "mdagm_back.cuh"
 #include "precond_tma.cuh"
 #include "measure_kernels.cuh"
+#include "cg_batched.cuh"
 
 namespace hqmc {
 
@@ -106,6 +107,15 @@ struct hqmc_ctx {
     bool ms_ready = false, ms_plan_ok = false;
     cufftHandle ms_plan = 0;
     void *d_ms_a = nullptr, *d_ms_b = nullptr, *d_ms_acc = nullptr;
+    // multi-right-hand-side PCG (hqmc_api_cgb.inl): workspace for cgb_cap vectors, created on first use
+    int cgb_cap = 0, cgb_pstride = 0;
+    void *d_cgb_r = nullptr, *d_cgb_d = nullptr, *d_cgb_Od = nullptr, *d_cgb_phi = nullptr;
+    double *d_cgb_part = nullptr;          // [5][cgb_cap][cgb_pstride]: dOd, rr, rz[0], rz[1], spare
+    hqmc::CgState *d_cgb_state = nullptr, *h_cgb_state = nullptr;
+    cudaGraphExec_t cgb_graph = nullptr;
+    void *cgb_graph_x = nullptr; int cgb_graph_n = 0, cgb_graph_tt = 0, cgb_graph_W = -1;
+    long long cgb_nodes[HQMC_K_COUNT] = {};
+    int green_batch = 0;                   // hqmc_set_green_batch: 0 = by footprint, 1 = one vector at a time, n = n at a time
     bool cg_defer_x;     // deferred-x PCG vector kernels (k_cg_raxpy + k_cg_xdupdate)
     int cg_chunk;            // iterations per graph launch
     // instrumentation

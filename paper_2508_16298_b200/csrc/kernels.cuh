@@ -58,6 +58,7 @@ __global__ void __launch_bounds__(MAXT) k_apply_M(Geo g, const typename Cx<T>::t
     BlockIdx b[BPT];
 #pragma unroll
     for (int k = 0; k < BPT; ++k) make_block(g, threadIdx.x + k * blockDim.x, b[k]);
+    in += (size_t)blockIdx.y * g.Vs * g.Nt; out += (size_t)blockIdx.y * g.Vs * g.Nt;   // blockIdx.y: vector of a batch
     const int tb = blockIdx.x, tnx = (tb + 1 == g.Nt) ? 0 : tb + 1;
     const int src = dagger ? tnx : tb, dst = dagger ? tb : tnx;
     const T sC = (tb == g.Nt - 1) ? C : -C;     // -sigma*C
@@ -88,9 +89,11 @@ __global__ void __launch_bounds__(MAXT) k_apply_M(Geo g, const typename Cx<T>::t
 template <typename T, int BPT, int MAXT, bool DOT>
 __global__ void __launch_bounds__(MAXT) k_mdagm(Geo g, int Tt, const typename Cx<T>::type *__restrict__ ph,
                         const typename Cx<T>::type *__restrict__ in, typename Cx<T>::type *__restrict__ out, T C,
-                        double *__restrict__ part, const CgState *__restrict__ st) {
+                        double *__restrict__ part, const CgState *__restrict__ st, int part_stride) {
     typedef typename Cx<T>::type T2;
-    if (st != nullptr && *(volatile const int *)&st->done) return;
+    // blockIdx.y: vector of a batch (cg_batched.cuh) with its own CgState and its own row of partials, part_stride apart
+    if (st != nullptr) { st += blockIdx.y; if (*(volatile const int *)&st->done) return; }
+    in += (size_t)blockIdx.y * g.Vs * g.Nt; out += (size_t)blockIdx.y * g.Vs * g.Nt;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Exch<T2> ex; ex.buf = reinterpret_cast<T2 *>(smem_raw); ex.nb = g.nb; ex.parity = 0;
     double *red = reinterpret_cast<double *>(smem_raw + sizeof(T2) * 4 * g.nb);
@@ -159,7 +162,7 @@ __global__ void __launch_bounds__(MAXT) k_mdagm(Geo g, int Tt, const typename Cx
     }
     if (DOT) {
         double s = block_sum(acc, red);
-        if (threadIdx.x == 0) part[blockIdx.x] = s;
+        if (threadIdx.x == 0) part[(size_t)blockIdx.y * part_stride + blockIdx.x] = s;
     }
 }
 

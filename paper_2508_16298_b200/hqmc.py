@@ -23,7 +23,7 @@ KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
-    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_cg_solve_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_fusion", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
@@ -203,6 +203,20 @@ class HQMC:
     def _vecs(self, v):
         assert v.is_cuda and v.dtype == self.cdtype and v.is_contiguous() and v.numel() % self.N == 0 and v.numel() >= self.N
         return v, v.numel() // self.N
+
+    def cg_solve_batched(self, rhs, tol=1e-10, max_iter=1000000, x=None):
+        """M^+M x_b = rhs_b for the stacked right-hand sides [n][Ntau][L][L], all advancing in the same launches
+        -> (x, iterations[n], relative recurrence residuals[n], all converged)."""
+        rhs, n = self._vecs(rhs)
+        x = torch.empty_like(rhs) if x is None else x
+        it, rel = (C.c_longlong * n)(), (C.c_double * n)()
+        s = _check(_lib.hqmc_cg_solve_batched(self._ctx, _ptr(rhs), _ptr(x), C.c_int(n), C.c_double(tol), C.c_longlong(max_iter),
+                                              it, rel), allow_noconv=True)
+        return x, list(it), list(rel), s == HQMC_OK
+
+    def set_green_batch(self, n: int):
+        """Vectors green_apply solves per launch (0 = by L2 footprint, 1 = one at a time)."""
+        _check(_lib.hqmc_set_green_batch(self._ctx, C.c_int(n)))
 
     def green_apply(self, xi, tol=1e-10, max_iter=1000000, out=None):
         """g_k = (M^+M)^{-1} M^+ xi_k for the stacked vectors xi [n_rv][Ntau][L][L] -> (g, total iterations, converged)."""
