@@ -112,6 +112,19 @@ int hqmc_leapfrog_trajectory(hqmc_ctx *ctx, double *d_theta, double *d_p, const 
                              double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
                              long long *cg_iters_out);
 
+/* n_chain independent trajectories advanced together (independent Markov chains on one lattice shape):
+ * d_theta, d_p: [n_chain][Ntau][2][L][L] fp64 in/out, d_pf: [n_chain][Ntau][L][L] complex, all device, caller-owned, 16-byte
+ * aligned.  Chain b evolves exactly as hqmc_leapfrog_trajectory would evolve (theta_b, p_b, phi_b); the launches carry the
+ * chain index (one phase-table, one multi-right-hand-side PCG and one force/kick launch sequence per leapfrog step for all
+ * chains), the per-chain link-phase tables and solutions live in library-owned workspace.  H0_out, H1_out, cg_iters_out:
+ * HOST arrays of n_chain entries (may be NULL).  The context's own theta (hqmc_set_theta) is neither used nor changed.
+ * Supported for L <= 48 and Ntau <= 4096, else HQMC_EINVAL.  HQMC_ENOCONV if any solve of any chain missed cg_tol. */
+int hqmc_leapfrog_trajectory_batched(hqmc_ctx *ctx, double *d_theta, double *d_p, const void *d_pf, int n_chain, int nsteps,
+                                     double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
+                                     long long *cg_iters_out);
+/* Pseudofermion refresh of the chains (PAPER.md:185 step i): phi_b = M^+(theta_b) eta_b.  d_eta and d_phi must not overlap. */
+int hqmc_refresh_batched(hqmc_ctx *ctx, const double *d_theta, const void *d_eta, void *d_phi, int n_chain);
+
 /* One HQMC update, steps (i)-(iv) of PAPER.md:185-201.  The random numbers are inputs (d_eta complex Gaussian with
  * <|eta|^2> = 1, d_p Gaussian with variance 1/2, u uniform in [0,1); reading C6), so the caller owns the generator:
  *   phi = M^+(theta) eta;  leapfrog trajectory of nsteps steps (as hqmc_leapfrog_trajectory);

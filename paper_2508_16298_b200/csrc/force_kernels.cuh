@@ -107,6 +107,10 @@ __global__ void __launch_bounds__(MAXT) k_force(Geo g, const typename Cx<T>::typ
     BlockIdx b[BPT];
 #pragma unroll
     for (int k = 0; k < BPT; ++k) make_block(g, threadIdx.x + k * blockDim.x, b[k]);
+    {   // blockIdx.y: chain of a batch (hqmc_api_mdb.inl), each with its own gauge field, phase table, solution and momenta
+        const size_t nv = (size_t)blockIdx.y * g.Vs * g.Nt;
+        ph += 2 * nv; X += nv; out += 2 * nv; theta += 2 * nv;
+    }
     const int t = blockIdx.x, tn = (t + 1 == g.Nt) ? 0 : t + 1;
     const double sigma = (t == g.Nt - 1) ? -1.0 : 1.0;
     const T sC = (T)(-sigma) * C;

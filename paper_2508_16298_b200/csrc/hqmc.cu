@@ -223,9 +223,9 @@ template <typename T> static int do_mdagm(hqmc_ctx *c, const void *in, void *out
         constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
         if (dot)
             return launch(c, HQMC_K_MDAGM, k_mdagm<T, B, M, true>, dim3(grid), dim3(c->cfg.threads), block_smem(c), c->g, Tt,
-                          (const T2 *)c->d_ph, (const T2 *)in, (T2 *)out, (T)c->C, c->d_part_dOd, st, 0);
+                          (const T2 *)c->d_ph, (const T2 *)in, (T2 *)out, (T)c->C, c->d_part_dOd, st, 0, (size_t)0);
         return launch(c, HQMC_K_MDAGM, k_mdagm<T, B, M, false>, dim3(grid), dim3(c->cfg.threads), block_smem(c), c->g, Tt,
-                      (const T2 *)c->d_ph, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st, 0);
+                      (const T2 *)c->d_ph, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st, 0, (size_t)0);
     });
 }
 
@@ -364,4 +364,5 @@ using namespace hqmc;
 #include "hqmc_api_cg.inl"
 #include "hqmc_api_cgb.inl"
 #include "hqmc_api_md.inl"
+#include "hqmc_api_mdb.inl"
 #include "hqmc_api_measure.inl"

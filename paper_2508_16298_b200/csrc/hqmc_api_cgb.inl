@@ -11,18 +11,23 @@ static int cgb_reserve(hqmc_ctx *c, int n) {
     if (n <= c->cgb_cap) return HQMC_OK;
     CUDA_TRY(cudaStreamSynchronize(c->stream));
     if (c->cgb_graph) { cudaGraphExecDestroy(c->cgb_graph); c->cgb_graph = nullptr; }
-    void **bufs[] = {&c->d_cgb_r, &c->d_cgb_d, &c->d_cgb_Od, &c->d_cgb_phi, (void **)&c->d_cgb_part, (void **)&c->d_cgb_state};
+    void **bufs[] = {&c->d_cgb_r, &c->d_cgb_d, &c->d_cgb_Od, &c->d_cgb_phi, (void **)&c->d_cgb_part, (void **)&c->d_cgb_state,
+                     &c->d_cgb_ph, (void **)&c->d_cgb_scal};
     for (auto p : bufs) if (*p) { cudaFree(*p); *p = nullptr; }
     if (c->h_cgb_state) { cudaFreeHost(c->h_cgb_state); c->h_cgb_state = nullptr; }
+    if (c->h_cgb_scal) { cudaFreeHost(c->h_cgb_scal); c->h_cgb_scal = nullptr; }
     c->cgb_cap = 0;
     c->cgb_pstride = HQMC_MAX_PART;
     const size_t vb = (size_t)n * c->N * c->esz;
-    const size_t sizes[] = {vb, vb, vb, vb, sizeof(double) * 5 * (size_t)n * c->cgb_pstride, sizeof(CgState) * (size_t)n};
-    for (int i = 0; i < 6; ++i) {
+    // d_cgb_phi doubles as the solution X of the chains' trajectories; d_cgb_ph: one link-phase table per chain
+    const size_t sizes[] = {vb, vb, vb, vb, sizeof(double) * 5 * (size_t)n * c->cgb_pstride, sizeof(CgState) * (size_t)n, 2 * vb,
+                            sizeof(double) * 8 * (size_t)n};
+    for (int i = 0; i < 8; ++i) {
         cudaError_t e = cudaMalloc(bufs[i], sizes[i]);
         if (e != cudaSuccess) { g_last_error = std::string("cudaMalloc (batched PCG workspace): ") + cudaGetErrorString(e); return HQMC_ENOMEM; }
     }
     if (cudaMallocHost((void **)&c->h_cgb_state, sizeof(CgState) * (size_t)n) != cudaSuccess) { g_last_error = "cudaMallocHost failed"; return HQMC_ENOMEM; }
+    if (cudaMallocHost((void **)&c->h_cgb_scal, sizeof(double) * 8 * (size_t)n) != cudaSuccess) { g_last_error = "cudaMallocHost failed"; return HQMC_ENOMEM; }
     c->cgb_cap = n;
     return HQMC_OK;
 }
@@ -82,13 +87,13 @@ template <typename T> static int cgb_precond(hqmc_ctx *c, int n, const CgbGrids 
 // rows of the partial-sum workspace
 static double *cgb_row(hqmc_ctx *c, int row) { return c->d_cgb_part + (size_t)row * c->cgb_cap * c->cgb_pstride; }
 
-template <typename T> static int cgb_iteration(hqmc_ctx *c, int n, const CgbGrids &G, void *x, int par) {
+template <typename T> static int cgb_iteration(hqmc_ctx *c, int n, const CgbGrids &G, void *x, int par, const void *ph, size_t ph_stride) {
     typedef typename Cx<T>::type T2;
     double *p_dOd = cgb_row(c, 0), *p_rr = cgb_row(c, 1), *p_rz[2] = {cgb_row(c, 2), cgb_row(c, 3)};
     HQ_TRY(with_cfg(c, [&](auto bpt, auto maxt) -> int {
         constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
         return launch(c, HQMC_K_MDAGM, k_mdagm<T, B, M, true>, dim3(G.gm, n), dim3(c->cfg.threads), block_smem(c), c->g, G.tt,
-                      (const T2 *)c->d_ph, (const T2 *)c->d_cgb_d, (T2 *)c->d_cgb_Od, (T)c->C, p_dOd, (const CgState *)c->d_cgb_state, c->cgb_pstride);
+                      (const T2 *)ph, (const T2 *)c->d_cgb_d, (T2 *)c->d_cgb_Od, (T)c->C, p_dOd, (const CgState *)c->d_cgb_state, c->cgb_pstride, ph_stride);
     }));
     HQ_TRY(launch(c, HQMC_K_AXPY, k_cgb_axpy<T>, dim3(G.ge, n), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_cgb_r, (const T2 *)c->d_cgb_d,
                   (const T2 *)c->d_cgb_Od, (const double *)p_rz[par], G.n_rz, (const double *)p_dOd, G.gm, p_rr, c->cgb_pstride,
@@ -98,8 +103,8 @@ template <typename T> static int cgb_iteration(hqmc_ctx *c, int n, const CgbGrid
                   (const double *)p_rz[par ^ 1], (const double *)p_rz[par], G.n_rz, c->cgb_pstride, 0, (const CgState *)c->d_cgb_state);
 }
 
-template <typename T> static int cgb_build_graph(hqmc_ctx *c, int n, const CgbGrids &G, void *x) {
-    if (c->cgb_graph && c->cgb_graph_x == x && c->cgb_graph_n == n && c->cgb_graph_tt == G.tt && c->cgb_graph_W == c->taps.W) return HQMC_OK;
+template <typename T> static int cgb_build_graph(hqmc_ctx *c, int n, const CgbGrids &G, void *x, const void *ph, size_t ph_stride) {
+    if (c->cgb_graph && c->cgb_graph_x == x && c->cgb_graph_ph == ph && c->cgb_graph_phs == ph_stride && c->cgb_graph_n == n && c->cgb_graph_tt == G.tt && c->cgb_graph_W == c->taps.W) return HQMC_OK;
     if (c->cgb_graph) { cudaGraphExecDestroy(c->cgb_graph); c->cgb_graph = nullptr; }
     long long saved[HQMC_K_COUNT];
     for (int i = 0; i < HQMC_K_COUNT; ++i) { saved[i] = c->graph_nodes[i]; c->graph_nodes[i] = 0; }
@@ -107,7 +112,7 @@ template <typename T> static int cgb_build_graph(hqmc_ctx *c, int n, const CgbGr
     CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
     c->capturing = true;
     int st = HQMC_OK;
-    for (int i = 0; i < c->cg_chunk && st == HQMC_OK; ++i) st = cgb_iteration<T>(c, n, G, x, i & 1);
+    for (int i = 0; i < c->cg_chunk && st == HQMC_OK; ++i) st = cgb_iteration<T>(c, n, G, x, i & 1, ph, ph_stride);
     c->capturing = false;
     cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
     for (int i = 0; i < HQMC_K_COUNT; ++i) { c->cgb_nodes[i] = c->graph_nodes[i]; c->graph_nodes[i] = saved[i]; }
@@ -116,12 +121,14 @@ template <typename T> static int cgb_build_graph(hqmc_ctx *c, int n, const CgbGr
     e = cudaGraphInstantiate(&c->cgb_graph, graph, 0);
     cudaGraphDestroy(graph);
     CUDA_TRY(e);
-    c->cgb_graph_x = x; c->cgb_graph_n = n; c->cgb_graph_tt = G.tt; c->cgb_graph_W = c->taps.W;
+    c->cgb_graph_x = x; c->cgb_graph_ph = ph; c->cgb_graph_phs = ph_stride; c->cgb_graph_n = n; c->cgb_graph_tt = G.tt; c->cgb_graph_W = c->taps.W;
     return HQMC_OK;
 }
 
+// ph / ph_stride: link-phase tables of the batch (stride 0: one gauge field shared by all vectors; 2N: one per vector)
 template <typename T> static int cgb_solve_t(hqmc_ctx *c, const void *rhs, void *x, int n, double tol, long long max_iter,
-                                             long long *iters_out, double *relres_out) {
+                                             long long *iters_out, double *relres_out, const void *ph = nullptr, size_t ph_stride = 0) {
+    if (!ph) ph = c->d_ph;
     typedef typename Cx<T>::type T2;
     HQ_TRY(cgb_reserve(c, n));
     CgbGrids G;
@@ -138,14 +145,14 @@ template <typename T> static int cgb_solve_t(hqmc_ctx *c, const void *rhs, void 
     HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cgb_dupdate<T>, dim3(G.ge, n), dim3(256), 0, c->N, (T2 *)c->d_cgb_d, (const T2 *)c->d_cgb_Od,
                   (const double *)p_rz0, (const double *)p_rz0, G.n_rz, c->cgb_pstride, 1, (const CgState *)c->d_cgb_state));
     const bool use_graph = !c->profiling;
-    if (use_graph) HQ_TRY(cgb_build_graph<T>(c, n, G, x));
+    if (use_graph) HQ_TRY(cgb_build_graph<T>(c, n, G, x, ph, ph_stride));
     long long launched = 0;
     while (true) {
         if (use_graph) {
             CUDA_TRY(cudaGraphLaunch(c->cgb_graph, c->stream));
             for (int i = 0; i < HQMC_K_COUNT; ++i) c->launches[i] += c->cgb_nodes[i];
         } else {
-            for (int i = 0; i < c->cg_chunk; ++i) HQ_TRY(cgb_iteration<T>(c, n, G, x, i & 1));
+            for (int i = 0; i < c->cg_chunk; ++i) HQ_TRY(cgb_iteration<T>(c, n, G, x, i & 1, ph, ph_stride));
         }
         launched += c->cg_chunk;
         CUDA_TRY(cudaMemcpyAsync(c->h_cgb_state, c->d_cgb_state, sizeof(CgState) * n, cudaMemcpyDeviceToHost, c->stream));

@@ -14,26 +14,28 @@ extern "C" int hqmc_force_boson(hqmc_ctx *c, double *d_out) {
                   c->prm.c_tau, c->prm.K, c->prm.compact);
 }
 
-// enqueue the reductions; results land in c->d_scal[0..2] = S_B, sum p^2, S_F
-static int enqueue_energies(hqmc_ctx *c, const double *d_p, const void *d_phi, const void *d_x, int slot0) {
-    HQ_TRY(launch(c, HQMC_K_MISC, k_action_boson, dim3(c->grid_ew), dim3(256), 0, c->g, (const double *)c->d_theta, c->prm.c_tau,
+// enqueue the reductions for the gauge field d_theta: d_out[0..2] = S_B, sum p^2, S_F = Re <phi, x>
+static int enqueue_energies_at(hqmc_ctx *c, const double *d_theta, const double *d_p, const void *d_phi, const void *d_x, double *d_out) {
+    HQ_TRY(launch(c, HQMC_K_MISC, k_action_boson, dim3(c->grid_ew), dim3(256), 0, c->g, d_theta, c->prm.c_tau,
                   c->prm.K, c->prm.compact, c->d_part_misc));
-    HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew, c->d_scal + slot0));
+    HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew, d_out));
     if (d_p) {
         HQ_TRY(launch(c, HQMC_K_MISC, k_reduce<double>, dim3(c->grid_ew), dim3(256), 0, 0, (size_t)2 * c->N, (const void *)d_p,
                       (const void *)nullptr, c->d_part_misc));
-        HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew,
-                      c->d_scal + slot0 + 1));
+        HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew, d_out + 1));
     }
     if (d_phi && d_x) {
         if (c->prm.prec == HQMC_C128)
             HQ_TRY(launch(c, HQMC_K_MISC, k_reduce<double>, dim3(c->grid_ew), dim3(256), 0, 1, c->N, d_phi, d_x, c->d_part_misc));
         else
             HQ_TRY(launch(c, HQMC_K_MISC, k_reduce<float>, dim3(c->grid_ew), dim3(256), 0, 1, c->N, d_phi, d_x, c->d_part_misc));
-        HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew,
-                      c->d_scal + slot0 + 2));
+        HQ_TRY(launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, c->grid_ew, d_out + 2));
     }
     return HQMC_OK;
+}
+// at the context's theta; results land in c->d_scal[slot0 .. slot0 + 2]
+static int enqueue_energies(hqmc_ctx *c, const double *d_p, const void *d_phi, const void *d_x, int slot0) {
+    return enqueue_energies_at(c, c->d_theta, d_p, d_phi, d_x, c->d_scal + slot0);
 }
 
 extern "C" int hqmc_energies(hqmc_ctx *c, const double *d_p, const void *d_phi, const void *d_x, double *SB, double *p2, double *SF) {

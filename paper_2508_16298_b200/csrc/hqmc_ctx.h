@@ -110,6 +110,7 @@ struct hqmc_ctx {
     // multi-right-hand-side PCG (hqmc_api_cgb.inl): workspace for cgb_cap vectors, created on first use
     int cgb_cap = 0, cgb_pstride = 0;
     void *d_cgb_r = nullptr, *d_cgb_d = nullptr, *d_cgb_Od = nullptr, *d_cgb_phi = nullptr;
+    void *d_cgb_ph = nullptr; double *d_cgb_scal = nullptr, *h_cgb_scal = nullptr; const void *cgb_graph_ph = nullptr; size_t cgb_graph_phs = 0;
     double *d_cgb_part = nullptr;          // [5][cgb_cap][cgb_pstride]: dOd, rr, rz[0], rz[1], spare
     hqmc::CgState *d_cgb_state = nullptr, *h_cgb_state = nullptr;
     cudaGraphExec_t cgb_graph = nullptr;

@@ -89,11 +89,13 @@ __global__ void __launch_bounds__(MAXT) k_apply_M(Geo g, const typename Cx<T>::t
 template <typename T, int BPT, int MAXT, bool DOT>
 __global__ void __launch_bounds__(MAXT) k_mdagm(Geo g, int Tt, const typename Cx<T>::type *__restrict__ ph,
                         const typename Cx<T>::type *__restrict__ in, typename Cx<T>::type *__restrict__ out, T C,
-                        double *__restrict__ part, const CgState *__restrict__ st, int part_stride) {
+                        double *__restrict__ part, const CgState *__restrict__ st, int part_stride,
+                        size_t ph_stride) {
     typedef typename Cx<T>::type T2;
     // blockIdx.y: vector of a batch (cg_batched.cuh) with its own CgState and its own row of partials, part_stride apart
     if (st != nullptr) { st += blockIdx.y; if (*(volatile const int *)&st->done) return; }
     in += (size_t)blockIdx.y * g.Vs * g.Nt; out += (size_t)blockIdx.y * g.Vs * g.Nt;
+    ph += (size_t)blockIdx.y * ph_stride;      // 0: the batch shares one gauge field; 2N: one field per vector (chains)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Exch<T2> ex; ex.buf = reinterpret_cast<T2 *>(smem_raw); ex.nb = g.nb; ex.parity = 0;
     double *red = reinterpret_cast<double *>(smem_raw + sizeof(T2) * 4 * g.nb);

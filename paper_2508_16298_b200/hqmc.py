@@ -23,7 +23,7 @@ KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
-    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_cg_solve_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_fusion", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
@@ -203,6 +203,26 @@ class HQMC:
     def _vecs(self, v):
         assert v.is_cuda and v.dtype == self.cdtype and v.is_contiguous() and v.numel() % self.N == 0 and v.numel() >= self.N
         return v, v.numel() // self.N
+
+    def refresh_batched(self, theta, eta, out=None):
+        """phi_b = M^+(theta_b) eta_b for stacked chains: theta [n][Ntau][2][L][L], eta [n][Ntau][L][L]."""
+        eta, n = self._vecs(eta)
+        assert theta.is_cuda and theta.dtype == torch.float64 and theta.is_contiguous() and theta.numel() == 2 * self.N * n
+        out = torch.empty_like(eta) if out is None else out
+        _check(_lib.hqmc_refresh_batched(self._ctx, _ptr(theta), _ptr(eta), _ptr(out), C.c_int(n)))
+        return out
+
+    def trajectory_batched(self, theta, p, phi, nsteps, eps, cg_tol=1e-10, cg_max_iter=1000000):
+        """n independent chains advanced together; theta, p [n][Ntau][2][L][L] are updated in place
+        -> dict(H0[n], H1[n], cg_iters[n], converged)."""
+        phi, n = self._vecs(phi)
+        for f in (theta, p):
+            assert f.is_cuda and f.dtype == torch.float64 and f.is_contiguous() and f.numel() == 2 * self.N * n
+        H0, H1, it = (C.c_double * n)(), (C.c_double * n)(), (C.c_longlong * n)()
+        s = _check(_lib.hqmc_leapfrog_trajectory_batched(self._ctx, _ptr(theta), _ptr(p), _ptr(phi), C.c_int(n), C.c_int(nsteps),
+                                                         C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter), H0, H1, it),
+                   allow_noconv=True)
+        return dict(H0=list(H0), H1=list(H1), cg_iters=list(it), converged=(s == HQMC_OK))
 
     def cg_solve_batched(self, rhs, tol=1e-10, max_iter=1000000, x=None):
         """M^+M x_b = rhs_b for the stacked right-hand sides [n][Ntau][L][L], all advancing in the same launches

@@ -136,3 +136,42 @@ def test_batched_pcg_rejects_what_it_cannot_run(hq):
     out, it, ok = g.green_apply(v, 1e-10, 10)    # falls back to one vector at a time
     assert ok and it == 0
     g.close()
+
+
+# ---- n independent chains advanced together (hqmc_leapfrog_trajectory_batched; Eq.16, 181 Eq.12) -----------
+@pytest.mark.parametrize("L,Nt,seed,n,nsteps,compact", [(4, 8, 0, 3, 4, True), (6, 10, 1, 2, 3, False), (12, 14, 2, 3, 2, True)])
+def test_batched_trajectories_match_oracle_per_chain(hq, L, Nt, seed, n, nsteps, compact):
+    """Every chain of the batch against the oracle's one-chain trajectory on its own seeded (theta, p, eta): H0, H1, dH to
+    1e-8, theta' and p' to 1e-10 (north_star; solves at 1e-13 on both sides, reading C17), then reversibility of the batch."""
+    kw = dict(c_tau=1.3, K=0.7, compact=compact)
+    o = orc.Oracle(L, Nt, **kw)
+    orc.set_threads(orc.max_threads())
+    g = hq.HQMC(L, Nt, **kw)
+    thetas = [inputs.theta_uniform(L, Nt, seed + 100 * b) for b in range(n)]
+    ps = [inputs.momenta(L, Nt, seed + 100 * b) for b in range(n)]
+    etas = [inputs.complex_gaussian((Nt, L, L), seed + 100 * b) for b in range(n)]
+    phis = [o.apply_Mdag(th, eta) for th, eta in zip(thetas, etas)]
+    refs = [o.trajectory(th, p, phi, nsteps, 0.05, cg_tol=1e-13) for th, p, phi in zip(thetas, ps, phis)]
+    dth, dp = dev(np.stack(thetas)), dev(np.stack(ps))
+    # refresh on the GPU: phi_b = M^+(theta_b) eta_b
+    dphi = g.refresh_batched(dth, dev(np.stack(etas)))
+    for b in range(n):
+        assert rel(dphi[b].cpu().numpy(), phis[b]) <= 1e-12, b
+    r = g.trajectory_batched(dth, dp, dphi, nsteps, 0.05, cg_tol=1e-13)
+    assert r["converged"]
+    TH, P = dth.cpu().numpy(), dp.cpu().numpy()
+    for b in range(n):
+        ref = refs[b]
+        assert abs(r["H0"][b] - ref["H0"]) <= 1e-8 and abs(r["H1"][b] - ref["H1"]) <= 1e-8, b
+        assert abs((r["H1"][b] - r["H0"][b]) - (ref["H1"] - ref["H0"])) <= 1e-8, b
+        assert np.abs(TH[b] - ref["theta"]).max() <= 1e-10 and np.abs(P[b] - ref["p"]).max() <= 1e-10, b
+    # the context's own theta is not involved: a one-chain run of chain 1 through the one-vector path gives the same numbers
+    t1, p1 = dev(thetas[1]), dev(ps[1])
+    r1 = g.trajectory(t1, p1, dev(phis[1]), nsteps, 0.05, cg_tol=1e-13)
+    assert abs(r1["H1"] - r["H1"][1]) <= 1e-8 and float((t1 - dth[1]).abs().max()) <= 1e-10
+    # reversibility of all chains at once: flip p, integrate back
+    dp.neg_()
+    g.trajectory_batched(dth, dp, dphi, nsteps, 0.05, cg_tol=1e-13)
+    assert np.abs(dth.cpu().numpy() - np.stack(thetas)).max() <= 1e-10
+    assert np.abs(dp.cpu().numpy() + np.stack(ps)).max() <= 1e-10
+    g.close()
