@@ -384,6 +384,10 @@ def run_trajectory(args):
     from paper_2508_16298_b200 import hqmc, inputs
     c = inputs.CONFIGS[args.config]
     L, Ntau = c["L"], c["Ntau"]
+    if args.L:                                               # the paper's shape at another size: V_s = L^2, N_tau = 10 L
+        L, Ntau = args.L, 10 * args.L
+    if args.chains:
+        return run_chains(args, L, Ntau, c["seed"])
     N = L * L * Ntau
     paper = args.theta == "paper"
     theta0 = inputs.theta_paper_regime(L, Ntau, c["seed"]) if paper else inputs.make_theta(args.config)
@@ -417,6 +421,51 @@ def run_trajectory(args):
                       "MdagM_Gsite_per_s": it * N / (ms * 1e-3) / 1e9,
                       "hbm_fraction_alg": bps * N * it / (ms * 1e-3) / 1e9 / peak, "peak_GBps": peak, "peak_source": peak_src,
                       "dH": dH}))
+    g.close()
+    return 0
+
+
+def run_chains(args, L, Ntau, seed):
+    """--mode trajectory --chains n1,n2,...: n independent Markov chains advanced together on one GPU
+    (hqmc_leapfrog_trajectory_batched), paper-regime fields (4 distinct heat-bath fields cycled over the chains; momenta and
+    pseudofermions differ per chain), PCG to --tol.  Reports ms per batch of trajectories and trajectories per second for
+    every chain count, next to the one-chain path (chains = 1 runs hqmc_leapfrog_trajectory)."""
+    import torch
+    from paper_2508_16298_b200 import hqmc, inputs
+    N = L * L * Ntau
+    counts = [int(x) for x in args.chains.split(",")]
+    nmax = max(counts)
+    fields = [inputs.theta_paper_regime(L, Ntau, seed + 17 * k) for k in range(min(4, nmax))]
+    g = hqmc.HQMC(L, Ntau, c_tau=80.0, K=1.0)
+    out = {}
+    for n in counts:
+        times, iters = [], []
+        for k in range(args.n_traj + 1):                          # first one is warm-up
+            th = torch.from_numpy(np.stack([fields[b % len(fields)] for b in range(n)])).cuda()
+            p = torch.from_numpy(np.stack([inputs.momenta(L, Ntau, seed + 1000 * k + b) for b in range(n)])).cuda()
+            eta = torch.from_numpy(np.stack([inputs.complex_gaussian((Ntau, L, L), seed + 1000 * k + b) for b in range(n)])).cuda()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            if n == 1:
+                g.set_theta(th[0])
+                phi = g.apply_Mdag(eta[0].contiguous())
+                r = g.trajectory(th[0], p[0], phi, args.md_steps, args.eps, cg_tol=args.tol, cg_max_iter=args.max_iter)
+                its = r["cg_iters"]
+            else:
+                phi = g.refresh_batched(th, eta)
+                r = g.trajectory_batched(th, p, phi, args.md_steps, args.eps, cg_tol=args.tol, cg_max_iter=args.max_iter)
+                its = sum(r["cg_iters"])
+            e1.record(); torch.cuda.synchronize()
+            assert r["converged"]
+            if k:
+                times.append(e0.elapsed_time(e1)); iters.append(its)
+        ms, it = float(np.mean(times)), float(np.mean(iters))
+        out[str(n)] = {"ms_per_batch": ms, "trajectories_per_s": n / (ms * 1e-3), "cg_iters_all_chains": it,
+                       "MdagM_Gsite_per_s": it * N / (ms * 1e-3) / 1e9}
+    print(json.dumps({"mode": "trajectory", "chains": out, "L": L, "Ntau": Ntau, "sites": N, "md_steps": args.md_steps, "eps": args.eps,
+                      "theta": "paper regime (c_tau=80, K=1 heat bath, cold start), 4 fields cycled", "cg": f"to {args.tol:g}",
+                      "trajectories_timed": args.n_traj}))
     g.close()
     return 0
 
@@ -510,7 +559,8 @@ def main():
     ap.add_argument("--n-rv", type=int, default=40, help="measure mode: number of noise vectors (PAPER.md:244)")
     ap.add_argument("--green-batch", default="0", help="measure mode: vectors per launch of the batched PCG, comma list to compare "
                     "(0 = library default, 1 = one at a time); the first entry is the one the other stages run after")
-    ap.add_argument("--L", type=int, default=0, help="measure mode: lattice size override (N_tau = 10 L)")
+    ap.add_argument("--L", type=int, default=0, help="measure / trajectory modes: lattice size override (N_tau = 10 L)")
+    ap.add_argument("--chains", default="", help="trajectory mode: comma list of chain counts advanced together (paper-regime fields)")
     ap.add_argument("--tol", type=float, default=1e-10)
     ap.add_argument("--theta", default="config", choices=["config", "paper"], help="solve / trajectory modes: the config's field or a paper-regime field")
     ap.add_argument("--max-iter", type=int, default=3000000)
