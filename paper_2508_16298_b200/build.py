@@ -9,8 +9,14 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhqmc.so")
 SOURCES = ["hqmc.cu"]
-DEPS = ["block_engine.cuh", "kernels.cuh", "mdagm_stream.cuh", "tma.cuh", "mdagm_ws.cuh", "mdagm_cluster.cuh", "mdagm_back.cuh", "precond_tma.cuh", "measure_kernels.cuh", "cg_kernels.cuh", "force_kernels.cuh", "hqmc_ctx.h", "hqmc_api_setup.inl",
-        "hqmc_api_cg.inl", "hqmc_api_md.inl", "hqmc_api_measure.inl", os.path.join("..", "..", "include", "hqmc.h")]
+HEADER = os.path.join("..", "..", "include", "hqmc.h")
+
+
+def deps():
+    """Every header / include file of csrc (the single translation unit hqmc.cu includes them all) and the public header."""
+    return [f for f in sorted(os.listdir(CSRC)) if f.endswith((".cuh", ".h", ".inl"))] + [HEADER]
+
+
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "-shared", "--expt-relaxed-constexpr", "-cudart", "static",
               "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]      # cuFFT: the FFT of Eq.19 (library primitive)
@@ -20,7 +26,7 @@ def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + DEPS)
+    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + deps())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

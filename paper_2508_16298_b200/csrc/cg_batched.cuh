@@ -33,7 +33,7 @@ __global__ void k_cgb_init(size_t N, const typename Cx<T>::type *__restrict__ rh
 
 // alpha_b = <r,z>_b / <d,Od>_b;  x_b += alpha_b d_b;  r_b -= alpha_b Od_b;  part_rr = partial ||r_b||^2
 template <typename T>
-__global__ void k_cgb_axpy(size_t N, typename Cx<T>::type *__restrict__ x, typename Cx<T>::type *__restrict__ r,
+__global__ void __launch_bounds__(256, 8) k_cgb_axpy(size_t N, typename Cx<T>::type *__restrict__ x, typename Cx<T>::type *__restrict__ r,
                            const typename Cx<T>::type *__restrict__ d, const typename Cx<T>::type *__restrict__ Od,
                            const double *__restrict__ part_rz, int n_rz, const double *__restrict__ part_dOd, int n_dOd,
                            double *__restrict__ part_rr, int pstride, const CgState *__restrict__ st) {
@@ -48,10 +48,11 @@ __global__ void k_cgb_axpy(size_t N, typename Cx<T>::type *__restrict__ x, typen
     const T alpha = (T)(rz / dOd);
     double acc = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
-        T2 xi = x[i], ri = r[i], di = d[i], oi = Od[i];
+        // x is touched once per iteration: streamed (evict-first) so that r, d and Od|z of the whole batch stay L2-resident
+        T2 xi = __ldcs(x + i), ri = r[i], di = d[i], oi = Od[i];
         xi.x = fma(alpha, di.x, xi.x); xi.y = fma(alpha, di.y, xi.y);
         ri.x = fma(-alpha, oi.x, ri.x); ri.y = fma(-alpha, oi.y, ri.y);
-        x[i] = xi;
+        __stcs(x + i, xi);
         r[i] = ri;
         acc += (double)ri.x * (double)ri.x + (double)ri.y * (double)ri.y;
     }
@@ -182,7 +183,7 @@ __global__ void k_cgb_precond_gen(Geo g, Taps taps, const typename Cx<T>::type *
 
 // beta_b = <r,z>_new / <r,z>_old;  d_b = z_b + beta_b d_b   (first: d_b = z_b)
 template <typename T>
-__global__ void k_cgb_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, const typename Cx<T>::type *__restrict__ z,
+__global__ void __launch_bounds__(256, 8) k_cgb_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, const typename Cx<T>::type *__restrict__ z,
                               const double *__restrict__ part_new, const double *__restrict__ part_old, int n, int pstride,
                               int first, const CgState *__restrict__ st) {
     typedef typename Cx<T>::type T2;

@@ -34,9 +34,21 @@ static int cgb_reserve(hqmc_ctx *c, int n) {
 
 struct CgbGrids { int ge, gm, tt, pgx, pgy, pbs, ptr, n_rz; };
 
+// resident CTAs per SM of the register-ring preconditioner kernel for half bandwidth W (its ring of 2W+1 rows sets the registers)
+template <typename T> static int cgb_precond_occupancy(int W, int bs) {
+    int per_sm = 0;
+    switch (W) {
+#define HQ_CASE(w) case w: cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cgb_precond<T, w>, bs, 0); break;
+        HQ_CASE(1) HQ_CASE(2) HQ_CASE(3) HQ_CASE(4) HQ_CASE(5) HQ_CASE(6) HQ_CASE(7) HQ_CASE(8) HQ_CASE(9) HQ_CASE(10) HQ_CASE(11) HQ_CASE(12)
+#undef HQ_CASE
+        default: break;
+    }
+    return per_sm > 0 ? per_sm : 4;
+}
+
 template <typename T> static int cgb_grids(hqmc_ctx *c, int n, CgbGrids &G) {
-    // element-wise kernels: about eight 256-thread CTAs per SM over the whole batch
-    long long ge = (long long)((c->N + 255) / 256), cap = std::max<long long>(4, ((long long)c->n_sm * 8 + n - 1) / n);
+    // element-wise kernels: at most eight 256-thread CTAs per SM over the whole batch, so that the batch is ONE wave
+    long long ge = (long long)((c->N + 255) / 256), cap = std::max<long long>(4, ((long long)c->n_sm * 8) / n);
     G.ge = (int)std::min<long long>(std::min(ge, cap), HQMC_MAX_PART);
     // M^+M: one CTA per (run of tt slices, vector); tt = the shortest run that keeps the batch in one wave of resident CTAs
     int per_sm = 1;
@@ -54,7 +66,9 @@ template <typename T> static int cgb_grids(hqmc_ctx *c, int n, CgbGrids &G) {
     if (W >= 1 && W <= 12) {
         G.pgx = (Vs + 127) / 128;
         G.pbs = (((Vs + G.pgx - 1) / G.pgx) + 31) / 32 * 32;
-        long long tr = ((long long)n * G.pgx * Nt + (long long)c->n_sm * 8 - 1) / ((long long)c->n_sm * 8);
+        // runs just long enough for the whole batch to be ONE wave of resident CTAs (a second wave costs more than the halo)
+        const long long slots = (long long)c->n_sm * cgb_precond_occupancy<T>(W, G.pbs);
+        long long tr = ((long long)n * G.pgx * Nt + slots - 1) / slots;
         tr = std::min<long long>(std::max<long long>(tr, 2 * W + 1), Nt);
         while ((long long)G.pgx * ((Nt + tr - 1) / tr) > HQMC_MAX_PART) ++tr;
         G.ptr = (int)tr; G.pgy = (Nt + G.ptr - 1) / G.ptr; G.n_rz = G.pgx * G.pgy;
@@ -191,8 +205,8 @@ extern "C" int hqmc_set_green_batch(hqmc_ctx *c, int n) {
 static int green_batch_size(const hqmc_ctx *c, int n_rv) {
     if (!cgb_supported(c)) return 1;
     if (c->green_batch > 0) return std::min(c->green_batch, n_rv);
-    // by footprint: while the live sets (x, r, d, Od|z per vector) of the whole batch stay L2-resident
-    const size_t per_vec = 5 * c->N * c->esz;
+    // by footprint: while the live sets (r, d, Od|z per vector; x is streamed) of the whole batch stay L2-resident
+    const size_t per_vec = 5 * c->N * c->esz;      // one vector of margin: measured best (L=24: 11 vectors 44.0, 14 vectors 46.4 ps per site)
     const long long fit = (long long)(c->l2_bytes / per_vec);
     return (int)std::max<long long>(1, std::min<long long>(fit, n_rv));
 }

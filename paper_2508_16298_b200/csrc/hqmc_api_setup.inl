@@ -274,6 +274,7 @@ extern "C" int hqmc_set_debug_skip(hqmc_ctx *c, unsigned mask) {
     if (!c) return HQMC_EINVAL;
     c->skip_mask = mask;
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+    if (c->cgb_graph) { cudaGraphExecDestroy(c->cgb_graph); c->cgb_graph = nullptr; }
     return HQMC_OK;
 }
 extern "C" int hqmc_set_pdl(hqmc_ctx *c, int on) {
