@@ -125,6 +125,14 @@ int hqmc_leapfrog_trajectory_batched(hqmc_ctx *ctx, double *d_theta, double *d_p
 /* Pseudofermion refresh of the chains (PAPER.md:185 step i): phi_b = M^+(theta_b) eta_b.  d_eta and d_phi must not overlap. */
 int hqmc_refresh_batched(hqmc_ctx *ctx, const double *d_theta, const void *d_eta, void *d_phi, int n_chain);
 
+/* One HQMC update of every chain, steps (i)-(iv) of PAPER.md:185-201, chain by chain what hqmc_hqmc_step does: d_eta
+ * [n_chain][Ntau][L][L] complex Gaussian, d_p [n_chain][...] Gaussian (device); u: HOST array of n_chain uniforms in [0,1).
+ * Chain b is accepted iff u[b] < min(1, exp(H0_b - H1_b)); rejected chains get their theta back; d_p holds the final momenta.
+ * H0_out, H1_out, accepted_out, cg_iters_out: HOST arrays of n_chain entries (may be NULL). */
+int hqmc_hqmc_step_batched(hqmc_ctx *ctx, double *d_theta, double *d_p, const void *d_eta, const double *u, int n_chain,
+                           int nsteps, double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
+                           int *accepted_out, long long *cg_iters_out);
+
 /* One HQMC update, steps (i)-(iv) of PAPER.md:185-201.  The random numbers are inputs (d_eta complex Gaussian with
  * <|eta|^2> = 1, d_p Gaussian with variance 1/2, u uniform in [0,1); reading C6), so the caller owns the generator:
  *   phi = M^+(theta) eta;  leapfrog trajectory of nsteps steps (as hqmc_leapfrog_trajectory);

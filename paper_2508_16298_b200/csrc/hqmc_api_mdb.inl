@@ -102,3 +102,46 @@ extern "C" int hqmc_refresh_batched(hqmc_ctx *c, const double *d_theta, const vo
     if (!cgb_supported(c)) { g_last_error = "batched trajectories need L <= 48 (one thread per 2x2 block) and Ntau <= 4096"; return HQMC_EINVAL; }
     return DISPATCH_T(c, refresh_batched_t<double>(c, d_theta, d_eta, d_phi, n_chain), refresh_batched_t<float>(c, d_theta, d_eta, d_phi, n_chain));
 }
+
+// One HQMC update of every chain, steps (i)-(iv) of PAPER.md:185-201, as hqmc_hqmc_step does for one: the random numbers are
+// inputs (d_eta, d_p on the device; u on the host, one uniform per chain).  Rejected chains get their theta back.
+extern "C" int hqmc_hqmc_step_batched(hqmc_ctx *c, double *d_theta, double *d_p, const void *d_eta, const double *u, int n_chain,
+                                      int nsteps, double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
+                                      int *accepted_out, long long *cg_iters_out) {
+    if (!c || !aligned16(d_theta) || !aligned16(d_p) || !aligned16(d_eta) || !u || n_chain < 1 || nsteps < 0 || cg_max_iter < 0) return HQMC_EINVAL;
+    if (!cgb_supported(c)) { g_last_error = "batched trajectories need L <= 48 (one thread per 2x2 block) and Ntau <= 4096"; return HQMC_EINVAL; }
+    const size_t tb = sizeof(double) * 2 * c->N;
+    HQ_TRY(cgb_reserve(c, n_chain));
+    // theta_0 of every chain (for the rejections) and the pseudofermions: library-owned, grown on demand
+    if (c->cgb_theta0_cap < n_chain) {
+        if (c->d_cgb_theta0) { CUDA_TRY(cudaStreamSynchronize(c->stream)); cudaFree(c->d_cgb_theta0); c->d_cgb_theta0 = nullptr; c->cgb_theta0_cap = 0; }
+        CUDA_TRY(cudaMalloc((void **)&c->d_cgb_theta0, tb * n_chain));
+        c->cgb_theta0_cap = n_chain;
+    }
+    if (c->d_cgb_pf_cap < n_chain) {
+        if (c->d_cgb_pf) { CUDA_TRY(cudaStreamSynchronize(c->stream)); cudaFree(c->d_cgb_pf); c->d_cgb_pf = nullptr; c->d_cgb_pf_cap = 0; }
+        CUDA_TRY(cudaMalloc(&c->d_cgb_pf, c->N * c->esz * n_chain));
+        c->d_cgb_pf_cap = n_chain;
+    }
+    CUDA_TRY(cudaMemcpyAsync(c->d_cgb_theta0, d_theta, tb * n_chain, cudaMemcpyDeviceToDevice, c->stream));
+    HQ_TRY(hqmc_refresh_batched(c, d_theta, d_eta, c->d_cgb_pf, n_chain));                        // (i)
+    std::vector<double> H0((size_t)n_chain), H1((size_t)n_chain);
+    int s = hqmc_leapfrog_trajectory_batched(c, d_theta, d_p, c->d_cgb_pf, n_chain, nsteps, eps, cg_tol, cg_max_iter, H0.data(),
+                                             H1.data(), cg_iters_out);                                  // (ii)
+    if (s != HQMC_OK && s != HQMC_ENOCONV) return s;
+    bool any_rej = false;
+    for (int b = 0; b < n_chain; ++b) {
+        double r = std::exp(H0[b] - H1[b]);
+        if (r > 1.0) r = 1.0;
+        const int acc = (u[b] < r) ? 1 : 0;                                                             // (iii)
+        if (!acc) {                                                                                     // (iv)
+            CUDA_TRY(cudaMemcpyAsync(d_theta + (size_t)b * 2 * c->N, c->d_cgb_theta0 + (size_t)b * 2 * c->N, tb, cudaMemcpyDeviceToDevice, c->stream));
+            any_rej = true;
+        }
+        if (H0_out) H0_out[b] = H0[b];
+        if (H1_out) H1_out[b] = H1[b];
+        if (accepted_out) accepted_out[b] = acc;
+    }
+    if (any_rej) CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return s;
+}

@@ -168,7 +168,7 @@ extern "C" int hqmc_destroy(hqmc_ctx *c) {
     if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
     if (c->cg_graph) cudaGraphExecDestroy(c->cg_graph);
     if (c->cgb_graph) cudaGraphExecDestroy(c->cgb_graph);
-    { void *bp[] = {c->d_cgb_r, c->d_cgb_d, c->d_cgb_Od, c->d_cgb_phi, c->d_cgb_part, c->d_cgb_state, c->d_cgb_ph, c->d_cgb_scal}; for (void *p : bp) if (p) cudaFree(p); }
+    { void *bp[] = {c->d_cgb_r, c->d_cgb_d, c->d_cgb_Od, c->d_cgb_phi, c->d_cgb_part, c->d_cgb_state, c->d_cgb_ph, c->d_cgb_scal, c->d_cgb_theta0, c->d_cgb_pf}; for (void *p : bp) if (p) cudaFree(p); }
     if (c->h_cgb_state) cudaFreeHost(c->h_cgb_state);
     if (c->h_cgb_scal) cudaFreeHost(c->h_cgb_scal);
     for (auto &ep : c->pending) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }

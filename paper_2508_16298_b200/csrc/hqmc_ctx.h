@@ -111,6 +111,7 @@ struct hqmc_ctx {
     int cgb_cap = 0, cgb_pstride = 0;
     void *d_cgb_r = nullptr, *d_cgb_d = nullptr, *d_cgb_Od = nullptr, *d_cgb_phi = nullptr;
     void *d_cgb_ph = nullptr; double *d_cgb_scal = nullptr, *h_cgb_scal = nullptr; const void *cgb_graph_ph = nullptr; size_t cgb_graph_phs = 0;
+    double *d_cgb_theta0 = nullptr; int cgb_theta0_cap = 0; void *d_cgb_pf = nullptr; int d_cgb_pf_cap = 0;   // hqmc_hqmc_step_batched
     double *d_cgb_part = nullptr;          // [5][cgb_cap][cgb_pstride]: dOd, rr, rz[0], rz[1], spare
     hqmc::CgState *d_cgb_state = nullptr, *h_cgb_state = nullptr;
     cudaGraphExec_t cgb_graph = nullptr;

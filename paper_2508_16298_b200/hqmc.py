@@ -23,7 +23,7 @@ KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
-    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_fusion", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
@@ -223,6 +223,18 @@ class HQMC:
                                                          C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter), H0, H1, it),
                    allow_noconv=True)
         return dict(H0=list(H0), H1=list(H1), cg_iters=list(it), converged=(s == HQMC_OK))
+
+    def hqmc_step_batched(self, theta, p, eta, u, nsteps, eps, cg_tol=1e-10, cg_max_iter=1000000):
+        """One HQMC update of n chains (refresh, trajectory, Metropolis with the uniforms u[n], restore on rejection)."""
+        eta, n = self._vecs(eta)
+        for f in (theta, p):
+            assert f.is_cuda and f.dtype == torch.float64 and f.is_contiguous() and f.numel() == 2 * self.N * n
+        assert len(u) == n
+        H0, H1, it, acc = (C.c_double * n)(), (C.c_double * n)(), (C.c_longlong * n)(), (C.c_int * n)()
+        s = _check(_lib.hqmc_hqmc_step_batched(self._ctx, _ptr(theta), _ptr(p), _ptr(eta), (C.c_double * n)(*[float(v) for v in u]),
+                                               C.c_int(n), C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter),
+                                               H0, H1, acc, it), allow_noconv=True)
+        return dict(H0=list(H0), H1=list(H1), accepted=[bool(a) for a in acc], cg_iters=list(it), converged=(s == HQMC_OK))
 
     def cg_solve_batched(self, rhs, tol=1e-10, max_iter=1000000, x=None):
         """M^+M x_b = rhs_b for the stacked right-hand sides [n][Ntau][L][L], all advancing in the same launches

@@ -175,3 +175,31 @@ def test_batched_trajectories_match_oracle_per_chain(hq, L, Nt, seed, n, nsteps,
     assert np.abs(dth.cpu().numpy() - np.stack(thetas)).max() <= 1e-10
     assert np.abs(dp.cpu().numpy() + np.stack(ps)).max() <= 1e-10
     g.close()
+
+
+def test_batched_hqmc_step_accepts_and_rejects_per_chain(hq):
+    """One HQMC update of three chains with the oracle's draws: with c_tau = K = 0 and eps = 0.15 the
+    trajectories have dH > 0 (test_gpu_parity.py), so u = 0.99 rejects (theta back bit for bit) and u = 0.0 accepts, chain by
+    chain, in one batch."""
+    L, Nt, seed, n = 4, 8, 0, 3
+    o = orc.Oracle(L, Nt, c_tau=0.0, K=0.0)
+    g = hq.HQMC(L, Nt, c_tau=0.0, K=0.0)
+    thetas = [inputs.theta_uniform(L, Nt, seed + 100 * b) for b in range(n)]
+    ps = [inputs.momenta(L, Nt, seed + 100 * b) for b in range(n)]
+    etas = [inputs.complex_gaussian((Nt, L, L), seed + 100 * b) for b in range(n)]
+    us = [0.99, 0.0, 0.99]
+    refs = [o.hqmc_step(thetas[b], ps[b], etas[b], us[b], 6, 0.15, cg_tol=1e-13) for b in range(n)]
+    dth, dp = dev(np.stack(thetas)), dev(np.stack(ps))
+    r = g.hqmc_step_batched(dth, dp, dev(np.stack(etas)), us, 6, 0.15, cg_tol=1e-13)
+    assert r["converged"] and r["accepted"] == [ref["accepted"] for ref in refs]
+    assert r["accepted"][1] and not all(r["accepted"])           # both branches are exercised
+    TH, P = dth.cpu().numpy(), dp.cpu().numpy()
+    for b in range(n):
+        ref = refs[b]
+        assert abs(r["H0"][b] - ref["H0"]) <= 1e-8 and abs((r["H1"][b] - r["H0"][b]) - (ref["H1"] - ref["H0"])) <= 1e-8, b
+        if ref["accepted"]:
+            assert np.abs(TH[b] - ref["theta"]).max() <= 1e-10, b
+        else:
+            assert np.array_equal(TH[b], thetas[b]), b
+        assert np.abs(P[b] - ref["p"]).max() <= 1e-10, b
+    g.close()
