@@ -73,8 +73,22 @@ extern "C" int hqmc_leapfrog_trajectory_batched(hqmc_ctx *c, double *d_theta, do
                                                 long long *cg_iters_out) {
     if (!c || !aligned16(d_theta) || !aligned16(d_p) || !aligned16(d_pf) || n_chain < 1 || nsteps < 0 || cg_max_iter < 0) return HQMC_EINVAL;
     if (!cgb_supported(c)) { g_last_error = "batched trajectories need L <= 48 (one thread per 2x2 block) and Ntau <= 4096"; return HQMC_EINVAL; }
-    return DISPATCH_T(c, traj_batched_t<double>(c, d_theta, d_p, d_pf, n_chain, nsteps, eps, cg_tol, cg_max_iter, H0_out, H1_out, cg_iters_out),
-                      traj_batched_t<float>(c, d_theta, d_p, d_pf, n_chain, nsteps, eps, cg_tol, cg_max_iter, H0_out, H1_out, cg_iters_out));
+    // the chains are independent: advance them in groups whose PCG live set stays L2-resident (the rule of hqmc_green_apply;
+    // hqmc_set_green_batch overrides), which also bounds the workspace
+    int bs = green_batch_size(c, n_chain);
+    { const int groups = (n_chain + bs - 1) / bs; bs = (n_chain + groups - 1) / groups; }   // even groups: fewer distinct graphs
+    int worst = HQMC_OK;
+    for (int k = 0; k < n_chain; k += bs) {
+        const int n = std::min(bs, n_chain - k);
+        double *th = d_theta + (size_t)k * 2 * c->N, *p = d_p + (size_t)k * 2 * c->N;
+        const void *pf = (const char *)d_pf + (size_t)k * c->N * c->esz;
+        double *h0 = H0_out ? H0_out + k : nullptr, *h1 = H1_out ? H1_out + k : nullptr;
+        long long *it = cg_iters_out ? cg_iters_out + k : nullptr;
+        const int st = DISPATCH_T(c, traj_batched_t<double>(c, th, p, pf, n, nsteps, eps, cg_tol, cg_max_iter, h0, h1, it),
+                                  traj_batched_t<float>(c, th, p, pf, n, nsteps, eps, cg_tol, cg_max_iter, h0, h1, it));
+        if (st == HQMC_ENOCONV) worst = st; else if (st != HQMC_OK) return st;
+    }
+    return worst;
 }
 
 // phi_b = M^+(theta_b) eta_b for the chains (PAPER.md:185 step i): fills the per-chain phase tables from d_theta first

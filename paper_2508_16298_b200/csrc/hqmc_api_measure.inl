@@ -79,7 +79,8 @@ extern "C" int hqmc_green_apply(hqmc_ctx *c, const void *d_xi, void *d_g, int n_
     if (!c || !c->theta_set || !d_xi || !d_g || d_xi == d_g || n_rv < 1 || max_iter < 0 || !aligned16(d_xi) || !aligned16(d_g)) return HQMC_EINVAL;
     long long total = 0;
     int worst = HQMC_OK;
-    const int bs = green_batch_size(c, n_rv);
+    int bs = green_batch_size(c, n_rv);
+    { const int groups = (n_rv + bs - 1) / bs; bs = (n_rv + groups - 1) / groups; }      // even groups: fewer distinct graphs
     if (bs > 1) {                                  // several vectors per launch (hqmc_api_cgb.inl)
         std::vector<long long> its((size_t)bs);
         for (int k = 0; k < n_rv; k += bs) {
