@@ -309,11 +309,49 @@ def run_gpu(args):
             "cg_us_per_iter": us_per_iter, "cg_iters_per_s": 1e6 / us_per_iter, "cg_ms_per_solve_fixed": us_per_iter * I * 1e-3,
             "ms_per_trajectory_step": ms_per_step, "kernels": per_kernel, "mdagm_sweep": sweep,
             "dH": r["H1"] - r["H0"]}
+    if world == 1 and not args.no_small:
+        line["batched_chains"] = small_lattice_chains(torch, hqmc, inputs, args.cg_iters)
     print(json.dumps(line))
     g.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def small_lattice_chains(torch, hqmc, inputs, cg_iters, L=16, n_chain=40, md_steps=3, eps=0.01):
+    """Extra key of the JSON line (not the metric): a lattice that cannot fill the GPU on its own (L=16, N_tau=160) run as one
+    chain (hqmc_leapfrog_trajectory) and as n_chain independent chains advanced together (hqmc_leapfrog_trajectory_batched);
+    same protocol as the main step (uniform theta, fixed-count PCG).  Trajectories per second and all-in Gsite/s."""
+    try:
+        Ntau, N = 10 * L, L * L * 10 * L
+        g = hqmc.HQMC(L, Ntau)
+        th0 = np.stack([inputs.theta_uniform(L, Ntau, 100 + b) for b in range(n_chain)])
+        p0 = np.stack([inputs.momenta(L, Ntau, 100 + b) for b in range(n_chain)])
+        eta = torch.from_numpy(np.stack([inputs.complex_gaussian((Ntau, L, L), 100 + b) for b in range(n_chain)])).cuda()
+        out = {"L": L, "Ntau": Ntau, "md_steps": md_steps, "cg_iters_per_solve": cg_iters}
+        for n in (1, n_chain):
+            ms = []
+            for k in range(3):                                           # first one is warm-up
+                th, p = torch.from_numpy(th0[:n].copy()).cuda(), torch.from_numpy(p0[:n].copy()).cuda()
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                if n == 1:
+                    g.set_theta(th[0])
+                    r = g.trajectory(th[0], p[0], g.apply_Mdag(eta[0].contiguous()), md_steps, eps, cg_tol=0.0, cg_max_iter=cg_iters)
+                    its = r["cg_iters"]
+                else:
+                    r = g.trajectory_batched(th, p, g.refresh_batched(th, eta[:n].contiguous()), md_steps, eps, cg_tol=0.0, cg_max_iter=cg_iters)
+                    its = sum(r["cg_iters"])
+                e1.record(); torch.cuda.synchronize()
+                if k:
+                    ms.append(e0.elapsed_time(e1))
+            t = float(np.mean(ms))
+            out[f"chains_{n}"] = {"ms_per_batch": t, "trajectories_per_s": n / (t * 1e-3), "MdagM_Gsite_per_s": its * N / (t * 1e-3) / 1e9}
+        g.close()
+        return out
+    except Exception as e:                                               # never lose the metric line over the extra key
+        return {"error": repr(e)[:200]}
 
 
 def pcg_kernel_costs(g, torch, d_phi, iters):
@@ -551,6 +589,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--prec", default="c128", choices=["c128", "c64"])
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-small", action="store_true", help="skip the extra small-lattice batched-chains key of the JSON line")
     ap.add_argument("--mode", default="step", choices=["step", "solve", "measure", "trajectory"],
                     help="solve: one full PCG solve to --tol; measure: the stochastic estimator on a paper-regime field (neither is the timed metric)")
     ap.add_argument("--n-traj", type=int, default=5, help="trajectory mode: timed trajectories (BASELINE config 5: 5)")
