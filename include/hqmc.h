@@ -3,7 +3,7 @@
  * method of arxiv/paper_2508_16298 ("Scalable hybrid quantum Monte Carlo simulation of U(1) gauge
  * field coupled to fermions on GPU"), hand-written CUDA for sm_100a (NVIDIA B200).
  *
- * Citations are to /root/reference/PAPER.md (line numbers) and to the readings C1-C22 listed in
+ * Citations are to /root/reference/PAPER.md (line numbers) and to the readings C1-C24 listed in
  * DESIGN.md (taken from SURVEY.md section 8c).
  *
  * Conventions (all entry points)
@@ -53,7 +53,8 @@ typedef struct {
     hqmc_prec prec;    /* arithmetic of the fermion vectors                                        */
 } hqmc_params;
 
-/* Create a context for one lattice.  cuda_stream is a cudaStream_t (NULL = legacy default stream).
+/* Create a context for one lattice.  cuda_stream is a cudaStream_t; NULL = the library creates (and owns) a blocking
+ * stream of its own, which is ordered with the legacy default stream.
  * Allocates the workspace (phase table, theta copy, 5 CG vectors, scratch) and, if precond_W > 0,
  * builds the default preconditioner taps on the device from the library's own B at pi-flux
  * (reading C10: c_k = [B_pi^k]_00, p_m = sum_k c_k c_{k+m}). */
@@ -117,8 +118,10 @@ int hqmc_leapfrog_trajectory(hqmc_ctx *ctx, double *d_theta, double *d_p, const 
  * aligned.  Chain b evolves exactly as hqmc_leapfrog_trajectory would evolve (theta_b, p_b, phi_b); the launches carry the
  * chain index (one phase-table, one multi-right-hand-side PCG and one force/kick launch sequence per leapfrog step for all
  * chains), the per-chain link-phase tables and solutions live in library-owned workspace.  H0_out, H1_out, cg_iters_out:
- * HOST arrays of n_chain entries (may be NULL).  The context's own theta (hqmc_set_theta) is neither used nor changed.
- * Supported for L <= 48 and Ntau <= 4096, else HQMC_EINVAL.  HQMC_ENOCONV if any solve of any chain missed cg_tol. */
+ * HOST arrays of n_chain entries (may be NULL).  The context's own theta (hqmc_set_theta) is not used; call hqmc_set_theta
+ * again before the one-field entry points (where a batch of one would not pay -- one vector's PCG live set fills the L2,
+ * e.g. L = 48, Ntau = 480, or L > 48 -- the chains run one after the other on the one-chain kernels and overwrite it).
+ * HQMC_ENOCONV if any solve of any chain missed cg_tol. */
 int hqmc_leapfrog_trajectory_batched(hqmc_ctx *ctx, double *d_theta, double *d_p, const void *d_pf, int n_chain, int nsteps,
                                      double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
                                      long long *cg_iters_out);
@@ -162,9 +165,6 @@ int hqmc_green_apply(hqmc_ctx *ctx, const void *d_xi, void *d_g, int n_rv, doubl
  * block (L <= 48) and Ntau <= 4096, else HQMC_EINVAL.  Synchronises the stream.  HQMC_ENOCONV if any vector missed tol. */
 int hqmc_cg_solve_batched(hqmc_ctx *ctx, const void *d_rhs, void *d_x, int n_vec, double tol, long long max_iter,
                           long long *iters_out, double *relres_out);
-/* Vectors hqmc_green_apply solves per launch: 0 (default) = as many as keep the batch's live set L2-resident, 1 = one at a
- * time on the one-vector kernels, n > 1 = n at a time. */
-int hqmc_set_green_batch(hqmc_ctx *ctx, int n);
 
 /* Eq.17-19: C(Delta) = (1/N) sum_i a_i b_{i+Delta} = (1/N) F^{-1}[F[a]_{-k} F[b]_k](Delta), i + Delta periodic in tau, y and
  * x (reading C23), N = L*L*Ntau.  d_C may alias d_a or d_b. */
@@ -190,41 +190,8 @@ int hqmc_leapfrog_trajectory_host(hqmc_ctx *ctx, double *h_theta, double *h_p, c
                                   double eps, double cg_tol, long long cg_max_iter, double *H0_out,
                                   double *H1_out, long long *cg_iters_out);
 
-/* Instrumentation.  hqmc_set_profiling(ctx, 1) makes the library bracket each launch of its kernels
- * with CUDA events on the context's stream (CG then runs without graph replay); hqmc_get_kernel_stats
- * returns, for kernel class `which` (HQMC_K_*), the number of launches and the summed device time in
- * ms since the last hqmc_reset_stats.  Launch counts are kept even when profiling is off. */
-enum { HQMC_K_MDAGM = 0, HQMC_K_AXPY = 1, HQMC_K_PRECOND = 2, HQMC_K_DUPDATE = 3, HQMC_K_M = 4,
-       HQMC_K_FORCE = 5, HQMC_K_PHASE = 6, HQMC_K_MISC = 7, HQMC_K_COUNT = 8 };
-int hqmc_set_profiling(hqmc_ctx *ctx, int on);
-int hqmc_reset_stats(hqmc_ctx *ctx);
-int hqmc_get_kernel_stats(hqmc_ctx *ctx, int which, long long *launches_out, double *ms_out);
-/* Tuning knobs.  hqmc_set_time_tile: slices per CTA of the fused M^+M kernel (0 = library default: one CTA per SM
- * with the slices dealt out evenly).  hqmc_set_mdagm_kernel: 0 = streaming kernel (TMA bulk copies, packed link
- * phases; default where its staging buffers fit one SM: L <= 48 in complex128), 1 = register-only kernel,
- * 2 = warp-specialised strip-decoupled streaming kernel, 3 = cluster kernel (the slice split over 2/4/8 SMs with
- * distributed shared memory; default where one SM cannot hold the slice, e.g. L = 64 in complex128), 4 = streaming
- * kernel that sweeps its time run backwards (fewer live registers, third v buffer), 5 = the same with the halo
- * product handed over between neighbouring CTAs instead of recomputed. */
-int hqmc_set_time_tile(hqmc_ctx *ctx, int slices_per_cta);
-int hqmc_set_mdagm_kernel(hqmc_ctx *ctx, int which);
-/* Preconditioner kernel for W = 1..6: n > 0: TMA-tiled kernel, runs of n slices per CTA; n < 0: register-ring
- * kernel with runs of -n slices; 0 = library default (TMA-tiled). */
-int hqmc_set_precond_tile(hqmc_ctx *ctx, int slices_per_run);
-/* PCG vector kernels. 0 (default) = chosen by footprint: the textbook four kernels per iteration (M^+M | x += alpha d,
- * r -= alpha Od | z = P r | d = z + beta d) while the loop's live set (r, d, Od|z, packed phases) fits the L2, the deferred-x
- * four otherwise; 1 = fused residual-update + preconditioner and fused x/d update where the TMA-tiled preconditioner
- * applies (3 kernels per iteration); 2 = deferred-x forced (r -= alpha Od | z = P r | x += alpha d, d = z + beta d:
- * 16 B/site less traffic); 3 = textbook forced. All produce the same iterates. */
-int hqmc_set_cg_fusion(hqmc_ctx *ctx, int on);
-/* Programmatic dependent launch inside the PCG iteration (kernel k+1 is dispatched under kernel k's tail and waits
- * on-device for its completion before reading its output). 1 (default) = the preconditioner and the d update, the two
- * launches that follow a kernel filling every SM; 0 = off; 16 + mask = per-kernel-class mask (bit = HQMC_K_* class),
- * for timing experiments. Results are bit-identical in every setting. */
-int hqmc_set_pdl(hqmc_ctx *ctx, int on);
-/* TIMING ONLY: bit k of mask set = kernels of class HQMC_K_<k> are not launched (leave-one-out timing of a kernel
- * inside the graph-replayed PCG iteration; the numerical results are then meaningless).  0 restores normal operation. */
-int hqmc_set_debug_skip(hqmc_ctx *ctx, unsigned mask);
+/* Instrumentation and tuning knobs (launch statistics, kernel selection, timing experiments) are declared in
+ * hqmc_tuning.h; nothing in this header depends on them. */
 
 const char *hqmc_strerror(int status);
 const char *hqmc_last_error(void); /* text of the last CUDA error seen by this thread, or "" */

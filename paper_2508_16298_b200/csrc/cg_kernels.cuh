@@ -10,6 +10,11 @@
 
 namespace hqmc {
 
+// Device-side reset of the CG bookkeeping (no host buffer is read, so a solve can be replayed inside a CUDA graph).
+__global__ void k_cg_state_set(CgState *st, double tol2, long long max_iter) {
+    st->bb = 0.0; st->rr = 0.0; st->tol2 = tol2; st->iters = 0; st->max_iter = max_iter; st->done = 0; st->pad = 0;
+}
+
 // x = 0, r = rhs, part_rr[b] = partial ||rhs||^2
 template <typename T>
 __global__ void k_cg_init(size_t N, const typename Cx<T>::type *__restrict__ rhs, typename Cx<T>::type *__restrict__ x,
@@ -101,7 +106,7 @@ __global__ void k_precond(Geo g, Taps taps, const typename Cx<T>::type *__restri
             } else {
                 long long it = st->iters + 1;
                 st->iters = it; st->rr = rr;
-                if ((st->tol2 > 0.0 && rr <= st->tol2 * st->bb) || it >= st->max_iter) st->done = 1;
+                if ((st->tol2 > 0.0 && rr <= st->tol2 * st->bb) || it >= st->max_iter || rr != rr) st->done = 1;   // a non-finite residual stops the solve
             }
         }
     }
@@ -177,7 +182,7 @@ __global__ void __launch_bounds__(128) k_precond_win(Geo g, Taps taps, const typ
             } else {
                 long long it = st->iters + 1;
                 st->iters = it; st->rr = rr;
-                if ((st->tol2 > 0.0 && rr <= st->tol2 * st->bb) || it >= st->max_iter) st->done = 1;
+                if ((st->tol2 > 0.0 && rr <= st->tol2 * st->bb) || it >= st->max_iter || rr != rr) st->done = 1;   // a non-finite residual stops the solve
             }
         }
     }
@@ -208,7 +213,7 @@ __global__ void k_cg_dupdate(size_t N, typename Cx<T>::type *__restrict__ d, con
 }
 
 // ------------------------------------------------------------------------------------------------
-// Deferred-x form of the two vector kernels (opt-in, hqmc_set_cg_fusion(2)): x_{k+1} = x_k + alpha_k d_k is applied when d_k is read anyway
+// Deferred-x form of the two vector kernels (hqmc_set_cg_variant(HQMC_CG_DEFERRED_X); the default when the live set exceeds the L2): x_{k+1} = x_k + alpha_k d_k is applied when d_k is read anyway
 // to form d_{k+1}, so d is streamed once per iteration instead of twice (128 instead of 144 B/site for the pair):
 //   k_cg_raxpy   :  alpha = <r,z>/<d,Od>;  r -= alpha Od;  partial ||r||^2                      (48 B/site)
 //   k_cg_xdupdate:  x += alpha d;  beta = <r,z>_new/<r,z>_old;  d = z + beta d                 (80 B/site)

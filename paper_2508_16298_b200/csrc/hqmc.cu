@@ -27,8 +27,8 @@ static int launch(hqmc_ctx *c, int kclass, void (*kernel)(KArgs...), dim3 grid, 
     const bool use_pdl = c->pdl_next && ((c->pdl >> kclass) & 1);
     c->pdl_next = false;
     if (c->skip_mask & (1u << kclass)) return HQMC_OK;   // leave-one-out timing (results are then meaningless)
-    if (c->capturing) c->graph_nodes[kclass]++; else c->launches[kclass]++;
-    const bool prof = c->profiling && !c->capturing;
+    if (c->capturing) c->graph_nodes[kclass]++; else if (c->capturing_md) c->md_nodes_cur[kclass]++; else c->launches[kclass]++;
+    const bool prof = c->profiling && !c->capturing && !c->capturing_md;
     EventPair ep{};
     if (prof) {
         if (c->pending.size() >= 2048) HQ_TRY(drain_events(c));
@@ -38,7 +38,7 @@ static int launch(hqmc_ctx *c, int kclass, void (*kernel)(KArgs...), dim3 grid, 
         CUDA_TRY(cudaEventRecord(ep.a, c->stream));
     }
     if (use_pdl) {
-        // programmatic dependent launch: the PCG kernels call griddepcontrol.launch_dependents at their top and
+        // programmatic dependent launch: the PCG kernels call griddepcontrol.launch_dependents at their TAIL and
         // griddepcontrol.wait before touching anything the previous kernel wrote, so the launch latency of kernel k+1
         // (and, for M^+M, its barrier set-up and table fetch) hides under kernel k instead of adding to the iteration
         cudaLaunchConfig_t cfg = {};
@@ -81,18 +81,8 @@ template <typename T> static int set_attrs(hqmc_ctx *c) {
         CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, false>, attr, smem));
         CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, true>, attr, smem));
         if (c->use_stream) {
-            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_stream<T, false>, attr, (int)c->stream_smem));
-            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_stream<T, true>, attr, (int)c->stream_smem));
-        }
-        if (c->use_back) {
-            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, false, false>, attr, (int)c->back_smem));
-            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, true, false>, attr, (int)c->back_smem));
-            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, false, true>, attr, (int)c->back_smem));
-            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, true, true>, attr, (int)c->back_smem));
-        }
-        if (c->use_ws) {
-            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_ws<T, false>, attr, (int)c->ws_smem));
-            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_ws<T, true>, attr, (int)c->ws_smem));
+            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, false>, attr, (int)c->stream_smem));
+            CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, true>, attr, (int)c->stream_smem));
         }
         return HQMC_OK;
     });
@@ -143,35 +133,20 @@ template <typename T> static int do_mdagm_stream(hqmc_ctx *c, const void *in, vo
     typedef typename PhasePack<T>::word W;
     int G = c->time_tile > 0 ? (c->g.Nt + c->time_tile - 1) / c->time_tile : (c->g.Nt < c->n_sm ? c->g.Nt : c->n_sm);
     c->grid_mdagm = G;
-    if (c->use_back && c->back_on) {
-        auto go = [&](auto kern, double *part) -> int {
-            c->pdl_next = true;                       // k_mdagm_back calls griddepcontrol.wait
-            return launch(c, HQMC_K_MDAGM, kern, dim3(G), dim3(c->cfg.threads), c->back_smem, c->g, (const W *)c->d_packed,
-                          (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, part, st, (T2 *)c->d_halo, c->d_flags);
-        };
-        if (c->back_coop) return dot ? go(k_mdagm_back<T, true, true>, c->d_part_dOd) : go(k_mdagm_back<T, false, true>, (double *)nullptr);
-        return dot ? go(k_mdagm_back<T, true, false>, c->d_part_dOd) : go(k_mdagm_back<T, false, false>, (double *)nullptr);
-    }
-    if (c->use_ws && c->ws_on) {
-        if (dot)
-            return launch(c, HQMC_K_MDAGM, k_mdagm_ws<T, true>, dim3(G), dim3(c->cfg.threads + 32), c->ws_smem, c->g,
-                          (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, c->d_part_dOd, st);
-        return launch(c, HQMC_K_MDAGM, k_mdagm_ws<T, false>, dim3(G), dim3(c->cfg.threads + 32), c->ws_smem, c->g,
-                      (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st);
-    }
+    c->pdl_next = true;                               // k_mdagm_back calls griddepcontrol.wait
     if (dot)
-        return launch(c, HQMC_K_MDAGM, k_mdagm_stream<T, true>, dim3(G), dim3(c->cfg.threads), c->stream_smem, c->g,
-                      (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, c->d_part_dOd, st);
-    return launch(c, HQMC_K_MDAGM, k_mdagm_stream<T, false>, dim3(G), dim3(c->cfg.threads), c->stream_smem, c->g,
-                  (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st);
+        return launch(c, HQMC_K_MDAGM, k_mdagm_back<T, true>, dim3(G), dim3(c->cfg.threads), c->stream_smem, c->g, (const W *)c->d_packed,
+                      (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, c->d_part_dOd, st);
+    return launch(c, HQMC_K_MDAGM, k_mdagm_back<T, false>, dim3(G), dim3(c->cfg.threads), c->stream_smem, c->g, (const W *)c->d_packed,
+                  (const double2 *)c->d_tab, (const T2 *)in, (T2 *)out, (T)c->C, (double *)nullptr, st);
 }
 
 // cluster launch (cudaLaunchKernelEx with a cluster dimension); same bookkeeping as launch()
 template <typename... KArgs, typename... Args>
 static int launch_cluster(hqmc_ctx *c, int kclass, void (*kernel)(KArgs...), int grid, int block, size_t smem, int R, Args... args) {
     if (c->skip_mask & (1u << kclass)) return HQMC_OK;
-    if (c->capturing) c->graph_nodes[kclass]++; else c->launches[kclass]++;
-    const bool prof = c->profiling && !c->capturing;
+    if (c->capturing) c->graph_nodes[kclass]++; else if (c->capturing_md) c->md_nodes_cur[kclass]++; else c->launches[kclass]++;
+    const bool prof = c->profiling && !c->capturing && !c->capturing_md;
     EventPair ep{};
     if (prof) {
         if (c->pending.size() >= 2048) HQ_TRY(drain_events(c));
@@ -258,34 +233,6 @@ static void precond_cfg(hqmc_ctx *c, int tile) {
     if (c->pc_kind == 0) { c->pc_tile = 0; c->pc_gx = c->grid_ew; c->pc_gy = 1; c->n_part_rz = c->grid_ew; return; }
     c->pc_tile = tile; c->pc_gx = gx; c->pc_gy = (c->g.Nt + tile - 1) / tile; c->n_part_rz = c->pc_gx * c->pc_gy;
     if (c->pc_kind == 2) c->pc_smem = (size_t)(tile + 2 * W) * 128 * c->esz;
-    // fused PCG kernels: 64-site tiles of r and Od
-    c->cg_fused = false;
-    if (c->pc_kind == 2 && c->fused_allowed) {
-        c->f_gx = (c->g.Vs + 63) / 64; c->f_gy = c->pc_gy; c->n_part_f = c->f_gx * c->f_gy;
-        c->f_smem = (size_t)2 * (tile + 2 * W) * 64 * c->esz;
-        c->cg_fused = W <= 6 && c->n_part_f <= HQMC_MAX_PART && c->f_smem <= 200 * 1024 && tile <= 24;   // <= 6 thread rows of 64
-    }
-}
-
-template <typename T, int W> static int launch_cg_rz(hqmc_ctx *c, const void *rin, void *rout, const double *rz_old, double *rz_new) {
-    typedef typename Cx<T>::type T2;
-    CUDA_TRY(cudaFuncSetAttribute(k_cg_rz<T, W, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->f_smem));
-    return launch(c, HQMC_K_PRECOND, k_cg_rz<T, W, 64>, dim3(c->f_gx, c->f_gy), dim3(64, (c->pc_tile + 3) / 4), c->f_smem, c->g, c->taps, (const T2 *)rin,
-                  (const T2 *)c->d_Od, (T2 *)rout, (T2 *)c->d_z, rz_old, c->n_part_f, (const double *)c->d_part_dOd, c->grid_mdagm,
-                  c->d_part_rr, rz_new, (const CgState *)c->d_state, c->pc_tile);
-}
-template <typename T> static int do_cg_rz(hqmc_ctx *c, const void *rin, void *rout, const double *rz_old, double *rz_new) {
-    switch (c->taps.W) {
-        case 1: return launch_cg_rz<T, 1>(c, rin, rout, rz_old, rz_new);
-        case 2: return launch_cg_rz<T, 2>(c, rin, rout, rz_old, rz_new);
-        case 3: return launch_cg_rz<T, 3>(c, rin, rout, rz_old, rz_new);
-        case 4: return launch_cg_rz<T, 4>(c, rin, rout, rz_old, rz_new);
-        case 5: return launch_cg_rz<T, 5>(c, rin, rout, rz_old, rz_new);
-        case 6: return launch_cg_rz<T, 6>(c, rin, rout, rz_old, rz_new);
-        default: break;
-    }
-    g_last_error = "fused PCG kernels need W in 1..6";
-    return HQMC_EINVAL;
 }
 
 template <typename T, int W> static int launch_precond_win(hqmc_ctx *c, const void *in, void *out, double *part_rz, int mode) {

@@ -7,18 +7,10 @@
 // into a no-op after convergence, so tolerance-based stopping and graph replay coexist.  The host looks
 // at the flag once per chunk.
 
-// Fused form (W = 1..6): [O d + <d,Od>] [r' = r - alpha Od, z = P r', ||r'||^2, <r',z>] [x += alpha d, d = z + beta d,
-// bookkeeping] -- 3 kernels, r ping-pongs between two buffers (iteration parity = `par`).
+// Deferred-x form (chosen when the loop's live set exceeds the L2): [O d] [r -= alpha Od] [z = P r] [x += alpha d, d = z + beta d].
 template <typename T> static int cg_iteration(hqmc_ctx *c, void *x, int par) {
     typedef typename Cx<T>::type T2;
     HQ_TRY(do_mdagm<T>(c, c->d_d, c->d_Od, true, c->d_state));
-    if (c->cg_fused) {
-        void *rin = par ? c->d_r2 : c->d_r, *rout = par ? c->d_r : c->d_r2;
-        HQ_TRY(do_cg_rz<T>(c, rin, rout, (const double *)c->d_part_rz[par], c->d_part_rz[par ^ 1]));
-        return launch(c, HQMC_K_DUPDATE, k_cg_xd<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)x, (T2 *)c->d_d, (const T2 *)c->d_z,
-                      (const double *)c->d_part_rz[par], (const double *)c->d_part_rz[par ^ 1], c->n_part_f,
-                      (const double *)c->d_part_dOd, c->grid_mdagm, (const double *)c->d_part_rr, c->d_state);
-    }
     // O d is dead once r has been updated, so z = P r is written over it: the iteration's live set is x, r, d, (Od|z) and
     // the packed phases, 88 MB at config 4, and stays largely L2-resident.
     void *zb = c->d_Od;
@@ -46,7 +38,7 @@ template <typename T> static int cg_iteration(hqmc_ctx *c, void *x, int par) {
 }
 
 template <typename T> static int cg_build_graph(hqmc_ctx *c, void *x) {
-    if (c->cg_graph && c->cg_graph_x == x && c->cg_graph_tile == c->time_tile && c->cg_graph_fused == c->cg_fused && c->cg_graph_defer == c->cg_defer_x) return HQMC_OK;
+    if (c->cg_graph && c->cg_graph_x == x && c->cg_graph_tile == c->time_tile && c->cg_graph_defer == c->cg_defer_x) return HQMC_OK;
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     for (int i = 0; i < HQMC_K_COUNT; ++i) c->graph_nodes[i] = 0;
     cudaGraph_t graph = nullptr;
@@ -61,28 +53,40 @@ template <typename T> static int cg_build_graph(hqmc_ctx *c, void *x) {
     e = cudaGraphInstantiate(&c->cg_graph, graph, 0);
     cudaGraphDestroy(graph);
     CUDA_TRY(e);
+    c->cfg_epoch++;
     c->cg_graph_x = x;
     c->cg_graph_tile = c->time_tile;
-    c->cg_graph_fused = c->cg_fused;
     c->cg_graph_defer = c->cg_defer_x;
+    return HQMC_OK;
+}
+
+// x_0 = 0, r_0 = rhs, z_0 = P r_0, d_0 = z_0; bookkeeping reset on the device.  Enqueue only.
+template <typename T> static int cg_start(hqmc_ctx *c, const void *rhs, void *x, double tol, long long max_iter) {
+    typedef typename Cx<T>::type T2;
+    HQ_TRY(launch(c, HQMC_K_MISC, k_cg_state_set, dim3(1), dim3(1), 0, c->d_state, tol > 0.0 ? tol * tol : 0.0, max_iter));
+    HQ_TRY(launch(c, HQMC_K_MISC, k_cg_init<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (const T2 *)rhs, (T2 *)x, (T2 *)c->d_r,
+                  c->d_part_rr));
+    HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[0], 1));
+    return launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)c->d_z,
+                  (const double *)c->d_part_rz[0], (const double *)c->d_part_rz[0], c->n_part_rz, 1, (const CgState *)c->d_state);
+}
+
+// A whole fixed-count solve enqueued without any host round trip: start-up kernels + ceil(max_iter / chunk)
+// replays of the chunk graph (its kernels turn into no-ops once the device-side count is reached).  Capturable: inside a
+// stream capture the chunk graph becomes a child graph node.  cg_build_graph(c, x) must have been called before.
+template <typename T> static int cg_enqueue_fixed(hqmc_ctx *c, const void *rhs, void *x, long long max_iter) {
+    HQ_TRY(cg_start<T>(c, rhs, x, 0.0, max_iter));
+    const long long nchunk = (max_iter + c->cg_chunk - 1) / c->cg_chunk;
+    for (long long k = 0; k < nchunk; ++k) {
+        CUDA_TRY(cudaGraphLaunch(c->cg_graph, c->stream));
+        for (int i = 0; i < HQMC_K_COUNT; ++i) (c->capturing_md ? c->md_nodes_cur[i] : c->launches[i]) += c->graph_nodes[i];
+    }
     return HQMC_OK;
 }
 
 template <typename T> static int cg_solve_t(hqmc_ctx *c, const void *rhs, void *x, double tol, long long max_iter,
                                             long long *iters_out, double *relres_out) {
-    typedef typename Cx<T>::type T2;
-    // state
-    c->h_state->bb = 0.0; c->h_state->rr = 0.0; c->h_state->tol2 = tol > 0.0 ? tol * tol : 0.0;
-    c->h_state->iters = 0; c->h_state->max_iter = max_iter; c->h_state->done = 0; c->h_state->pad = 0;
-    CUDA_TRY(cudaMemcpyAsync(c->d_state, c->h_state, sizeof(CgState), cudaMemcpyHostToDevice, c->stream));
-    // x_0 = 0, r_0 = rhs, z_0 = P r_0, d_0 = z_0
-    if (c->cg_fused)   // the fused kernels sum n_part_f >= n_part_rz partials: the start-up kernel fills the first n_part_rz
-        CUDA_TRY(cudaMemsetAsync(c->d_part_rz[0], 0, sizeof(double) * HQMC_MAX_PART, c->stream));
-    HQ_TRY(launch(c, HQMC_K_MISC, k_cg_init<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (const T2 *)rhs, (T2 *)x, (T2 *)c->d_r,
-                  c->d_part_rr));
-    HQ_TRY(do_precond<T>(c, c->d_r, c->d_z, c->d_part_rz[0], 1));
-    HQ_TRY(launch(c, HQMC_K_DUPDATE, k_cg_dupdate<T>, dim3(c->grid_ew), dim3(256), 0, c->N, (T2 *)c->d_d, (const T2 *)c->d_z,
-                  (const double *)c->d_part_rz[0], (const double *)c->d_part_rz[0], c->n_part_rz, 1, (const CgState *)c->d_state));
+    HQ_TRY(cg_start<T>(c, rhs, x, tol, max_iter));
     const bool use_graph = !c->profiling;
     if (use_graph) HQ_TRY(cg_build_graph<T>(c, x));
     long long launched = 0;
@@ -103,7 +107,7 @@ template <typename T> static int cg_solve_t(hqmc_ctx *c, const void *rhs, void *
     const double rel = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
     if (iters_out) *iters_out = c->h_state->iters;
     if (relres_out) *relres_out = rel;
-    if (tol > 0.0 && rel > tol) return HQMC_ENOCONV;
+    if (rel != rel || (tol > 0.0 && !(rel <= tol))) return HQMC_ENOCONV;      // also a non-finite residual (x is then meaningless)
     return HQMC_OK;
 }
 

@@ -182,7 +182,7 @@ template <typename T> static int cgb_solve_t(hqmc_ctx *c, const void *rhs, void 
         const double rel = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
         if (iters_out) iters_out[b] = c->h_cgb_state[b].iters;
         if (relres_out) relres_out[b] = rel;
-        if (tol > 0.0 && rel > tol) st = HQMC_ENOCONV;
+        if (rel != rel || (tol > 0.0 && !(rel <= tol))) st = HQMC_ENOCONV;
     }
     return st;
 }

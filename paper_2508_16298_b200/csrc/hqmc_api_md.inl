@@ -55,6 +55,36 @@ static int kick(hqmc_ctx *c, double *d_p, double half_eps, int nkick) {
     return DISPATCH_T(c, do_force<double>(c, c->d_X, d_p, true, half_eps, nkick), do_force<float>(c, c->d_X, d_p, true, half_eps, nkick));
 }
 
+// Leapfrog step as ONE CUDA graph ("CUDA graph for the whole fermionic force computation"; north_star (b)):
+// drift + link-phase rebuild, a whole fixed-count PCG solve (start-up kernels + the chunk graph as child graph
+// nodes) and the fused force + kick.  which = 0: a middle step (closing half kick + opening one of the next step),
+// which = 1: the last step.  Only for fixed-count solves: a tolerance stop needs the host to look at the flag.
+template <typename T> static int md_step_enqueue(hqmc_ctx *c, double *d_p, const void *d_pf, double eps, long long iters, int nkick) {
+    HQ_TRY(do_phase<T>(c, d_p, 2.0 * eps));                                  // theta += 2 p eps
+    HQ_TRY(cg_enqueue_fixed<T>(c, d_pf, c->d_X, iters));
+    return do_force<T>(c, c->d_X, d_p, true, 0.5 * eps, nkick);
+}
+static int md_graph_get(hqmc_ctx *c, int which, double *d_p, const void *d_pf, double eps, long long iters) {
+    HQ_TRY(DISPATCH_T(c, cg_build_graph<double>(c, c->d_X), cg_build_graph<float>(c, c->d_X)));     // before the capture
+    hqmc_ctx::MdGraph &m = c->md[which];
+    if (m.exec && m.p == d_p && m.pf == d_pf && m.eps == eps && m.iters == iters && m.epoch == c->cfg_epoch) return HQMC_OK;
+    if (m.exec) { cudaGraphExecDestroy(m.exec); m.exec = nullptr; }
+    for (int i = 0; i < HQMC_K_COUNT; ++i) m.nodes[i] = 0;
+    cudaGraph_t graph = nullptr;
+    CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+    c->capturing_md = true; c->md_nodes_cur = m.nodes;
+    const int nkick = which ? 1 : 2;
+    int st = DISPATCH_T(c, md_step_enqueue<double>(c, d_p, d_pf, eps, iters, nkick), md_step_enqueue<float>(c, d_p, d_pf, eps, iters, nkick));
+    c->capturing_md = false; c->md_nodes_cur = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (st != HQMC_OK || e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return st != HQMC_OK ? st : HQMC_ECUDA; }
+    e = cudaGraphInstantiate(&m.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { m.exec = nullptr; cudaGetLastError(); return HQMC_ECUDA; }
+    m.p = d_p; m.pf = d_pf; m.eps = eps; m.iters = iters; m.epoch = c->cfg_epoch;
+    return HQMC_OK;
+}
+
 extern "C" int hqmc_leapfrog_trajectory(hqmc_ctx *c, double *d_theta, double *d_p, const void *d_pf, int nsteps, double eps,
                                         double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
                                         long long *cg_iters_out) {
@@ -71,8 +101,19 @@ extern "C" int hqmc_leapfrog_trajectory(hqmc_ctx *c, double *d_theta, double *d_
     CUDA_TRY(cudaMemsetAsync(c->d_scal, 0, sizeof(double) * 8, c->stream));
     HQ_TRY(solve());
     HQ_TRY(enqueue_energies(c, d_p, d_pf, c->d_X, 0));                      // H0 parts -> d_scal[0..2]
+    bool step_graph = c->md_graph && !c->md_graph_broken && !c->profiling && c->skip_mask == 0 && cg_tol <= 0.0 && cg_max_iter > 0;
     for (int n = 0; n < nsteps; ++n) {
         if (n == 0) HQ_TRY(kick(c, d_p, 0.5 * eps, 1));                     // p += F(theta_0) eps/2
+        if (step_graph) {
+            const int which = (n == nsteps - 1) ? 1 : 0;
+            if (md_graph_get(c, which, d_p, d_pf, eps, cg_max_iter) == HQMC_OK) {
+                CUDA_TRY(cudaGraphLaunch(c->md[which].exec, c->stream));
+                for (int i = 0; i < HQMC_K_COUNT; ++i) c->launches[i] += c->md[which].nodes[i];
+                total += cg_max_iter;
+                continue;
+            }
+            c->md_graph_broken = true; step_graph = false;                  // e.g. child-graph capture refused: plain launches
+        }
         HQ_TRY(DISPATCH_T(c, do_phase<double>(c, d_p, 2.0 * eps), do_phase<float>(c, d_p, 2.0 * eps)));   // theta += 2 p eps
         HQ_TRY(solve());
         HQ_TRY(kick(c, d_p, 0.5 * eps, (n == nsteps - 1) ? 1 : 2));         // closing half kick (+ opening one of step n+1)

@@ -72,10 +72,24 @@ extern "C" int hqmc_leapfrog_trajectory_batched(hqmc_ctx *c, double *d_theta, do
                                                 double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
                                                 long long *cg_iters_out) {
     if (!c || !aligned16(d_theta) || !aligned16(d_p) || !aligned16(d_pf) || n_chain < 1 || nsteps < 0 || cg_max_iter < 0) return HQMC_EINVAL;
-    if (!cgb_supported(c)) { g_last_error = "batched trajectories need L <= 48 (one thread per 2x2 block) and Ntau <= 4096"; return HQMC_EINVAL; }
     // the chains are independent: advance them in groups whose PCG live set stays L2-resident (the rule of hqmc_green_apply;
     // hqmc_set_green_batch overrides), which also bounds the workspace
-    int bs = green_batch_size(c, n_chain);
+    int bs = cgb_supported(c) ? green_batch_size(c, n_chain) : 1;
+    if (bs <= 1) {
+        // one vector's live set already fills the L2 (L = 48, Ntau = 480), or the slice needs more than one block per thread
+        // (L > 48): the tuned one-chain kernels (TMA streaming / cluster M^+M, tiled preconditioner, PDL) beat a batch of one,
+        // so the chains go through hqmc_leapfrog_trajectory one after the other.  The context's own theta is overwritten.
+        int worst1 = HQMC_OK;
+        for (int k = 0; k < n_chain; ++k) {
+            const int st = hqmc_leapfrog_trajectory(c, d_theta + (size_t)k * 2 * c->N, d_p + (size_t)k * 2 * c->N,
+                                                    (const char *)d_pf + (size_t)k * c->N * c->esz, nsteps, eps, cg_tol, cg_max_iter,
+                                                    H0_out ? H0_out + k : nullptr, H1_out ? H1_out + k : nullptr,
+                                                    cg_iters_out ? cg_iters_out + k : nullptr);
+            if (st == HQMC_ENOCONV) worst1 = st; else if (st != HQMC_OK) return st;
+        }
+        c->theta_set = false;                      // the context's phase tables now belong to the last chain
+        return worst1;
+    }
     { const int groups = (n_chain + bs - 1) / bs; bs = (n_chain + groups - 1) / groups; }   // even groups: fewer distinct graphs
     int worst = HQMC_OK;
     for (int k = 0; k < n_chain; k += bs) {
@@ -123,7 +137,18 @@ extern "C" int hqmc_hqmc_step_batched(hqmc_ctx *c, double *d_theta, double *d_p,
                                       int nsteps, double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
                                       int *accepted_out, long long *cg_iters_out) {
     if (!c || !aligned16(d_theta) || !aligned16(d_p) || !aligned16(d_eta) || !u || n_chain < 1 || nsteps < 0 || cg_max_iter < 0) return HQMC_EINVAL;
-    if (!cgb_supported(c)) { g_last_error = "batched trajectories need L <= 48 (one thread per 2x2 block) and Ntau <= 4096"; return HQMC_EINVAL; }
+    if (!cgb_supported(c) || green_batch_size(c, n_chain) <= 1) {           // see hqmc_leapfrog_trajectory_batched: one chain at a time
+        int worst1 = HQMC_OK;
+        for (int k = 0; k < n_chain; ++k) {
+            const int st = hqmc_hqmc_step(c, d_theta + (size_t)k * 2 * c->N, d_p + (size_t)k * 2 * c->N,
+                                          (const char *)d_eta + (size_t)k * c->N * c->esz, u[k], nsteps, eps, cg_tol, cg_max_iter,
+                                          H0_out ? H0_out + k : nullptr, H1_out ? H1_out + k : nullptr,
+                                          accepted_out ? accepted_out + k : nullptr, cg_iters_out ? cg_iters_out + k : nullptr);
+            if (st == HQMC_ENOCONV) worst1 = st; else if (st != HQMC_OK) return st;
+        }
+        c->theta_set = false;
+        return worst1;
+    }
     const size_t tb = sizeof(double) * 2 * c->N;
     HQ_TRY(cgb_reserve(c, n_chain));
     // theta_0 of every chain (for the rejections) and the pseudofermions: library-owned, grown on demand

@@ -100,7 +100,9 @@ extern "C" int hqmc_green_apply(hqmc_ctx *c, const void *d_xi, void *d_g, int n_
         char *g = (char *)d_g + (size_t)k * c->N * c->esz;
         HQ_TRY(DISPATCH_T(c, do_apply_M<double>(c, xi, c->d_phi, 1), do_apply_M<float>(c, xi, c->d_phi, 1)));     // R = M^+ xi
         long long it = 0;
-        const int st = cg_solve_any(c, c->d_phi, g, tol, max_iter, &it, nullptr);
+        // solve into the context's own X: the PCG graph (keyed on the solution pointer) is captured once, not once per vector
+        const int st = cg_solve_any(c, c->d_phi, c->d_X, tol, max_iter, &it, nullptr);
+        CUDA_TRY(cudaMemcpyAsync(g, c->d_X, c->N * c->esz, cudaMemcpyDeviceToDevice, c->stream));
         total += it;
         if (st == HQMC_ENOCONV) worst = st; else if (st != HQMC_OK) return st;
     }

@@ -64,9 +64,8 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     c->esz = (prm->prec == HQMC_C128) ? 16 : 8;
     c->own_stream = (cuda_stream == nullptr);
     c->stream = (cudaStream_t)cuda_stream;
-    c->cg_graph = nullptr; c->cg_graph_x = nullptr; c->cg_graph_tile = 0; c->cg_graph_fused = false; c->cg_graph_defer = false; c->cg_defer_x = false; c->cg_chunk = 32;
-    c->profiling = false; c->capturing = false; c->theta_set = false; c->skip_mask = 0; c->cg_fused = false; c->pdl = HQMC_PDL_DEFAULT; c->pdl_next = false;
-    c->fused_allowed = false;   // fused PCG vector kernels measured no faster at L=48: opt-in
+    c->cg_graph = nullptr; c->cg_graph_x = nullptr; c->cg_graph_tile = 0; c->cg_graph_defer = false; c->cg_defer_x = false; c->cg_chunk = 32;
+    c->profiling = false; c->capturing = false; c->theta_set = false; c->skip_mask = 0; c->pdl = HQMC_PDL_DEFAULT; c->pdl_next = false;
     for (int i = 0; i < HQMC_K_COUNT; ++i) { c->launches[i] = 0; c->graph_nodes[i] = 0; c->ms[i] = 0.0; }
     int st = HQMC_OK;
     auto fail = [&](int s) { hqmc_destroy(c); return s; };
@@ -98,19 +97,11 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     do { cudaError_t e = cudaMalloc((void **)&(ptr), (bytes));                                                    \
          if (e != cudaSuccess) { g_last_error = std::string("cudaMalloc: ") + cudaGetErrorString(e); return fail(HQMC_ENOMEM); } } while (0)
     ALLOC(c->d_theta, tb); ALLOC(c->d_ph, 2 * c->N * c->esz);
-    {   // streaming M^+M kernel: one thread per 2x2 block and its staging buffers must fit one SM's shared memory
-        const size_t need = (prm->prec == HQMC_C128) ? StreamSmem<double>(c->g.Vs, c->cfg.threads).total : StreamSmem<float>(c->g.Vs, c->cfg.threads).total;
+    {   // streaming M^+M kernel (k_mdagm_back): one thread per 2x2 block and its staging buffers must fit one SM's shared memory
+        const size_t need = (prm->prec == HQMC_C128) ? BackSmem<double>(c->g.Vs, c->cfg.threads).total : BackSmem<float>(c->g.Vs, c->cfg.threads).total;
         c->stream_smem = need;
         c->use_stream = (c->cfg.bpt == 1) && need <= (size_t)prop.sharedMemPerBlockOptin && (size_t)c->g.Vs * 16 < (1u << 20);
         c->stream_on = c->use_stream;
-        const int ws_ns = ws_geometry(h, c->cfg.threads).ns;
-        c->ws_smem = (prm->prec == HQMC_C128) ? WsSmem<double>(c->g.Vs, c->cfg.threads, h, ws_ns).total
-                                              : WsSmem<float>(c->g.Vs, c->cfg.threads, h, ws_ns).total;
-        c->use_ws = c->use_stream && c->cfg.threads + 32 <= 608 && c->ws_smem <= (size_t)prop.sharedMemPerBlockOptin;
-        c->ws_on = false;   // measured slower than k_mdagm_stream (profiles/): kept selectable
-        c->back_smem = (prm->prec == HQMC_C128) ? BackSmem<double>(c->g.Vs, c->cfg.threads).total : BackSmem<float>(c->g.Vs, c->cfg.threads).total;
-        c->use_back = c->use_stream && c->back_smem <= (size_t)prop.sharedMemPerBlockOptin;
-        c->back_on = c->use_back; c->back_coop = false;   // default: backward sweep, halo recomputed (hand-over measured slower)
         // cluster kernel: the slice split over R SMs (smallest R whose strip fits one SM's threads and shared memory)
         c->use_cluster = false; c->cluster_on = false; c->cl_R = 0;
         for (int R = 2; R <= 8 && !c->use_cluster; R *= 2) {
@@ -122,11 +113,6 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
             }
         }
         c->cluster_on = c->use_cluster && !c->use_stream;      // default only where one SM cannot hold the slice
-    }
-    if (c->use_back) {
-        ALLOC(c->d_halo, c->N * c->esz);
-        ALLOC(c->d_flags, sizeof(unsigned) * HQMC_MAX_PART);
-        cudaMemset(c->d_flags, 0, sizeof(unsigned) * HQMC_MAX_PART);
     }
     if (c->use_stream || c->use_cluster) {
         ALLOC(c->d_packed, 2 * c->N * 8);
@@ -141,7 +127,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
         cudaError_t e = cudaMemcpy(c->d_tab, tab.data(), sizeof(double2) * tab.size(), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) { g_last_error = cudaGetErrorString(e); return fail(HQMC_ECUDA); }
     }
-    ALLOC(c->d_r, vb); ALLOC(c->d_r2, vb); ALLOC(c->d_z, vb); ALLOC(c->d_d, vb); ALLOC(c->d_Od, vb); ALLOC(c->d_X, vb); ALLOC(c->d_phi, vb);
+    ALLOC(c->d_r, vb); ALLOC(c->d_z, vb); ALLOC(c->d_d, vb); ALLOC(c->d_Od, vb); ALLOC(c->d_X, vb); ALLOC(c->d_phi, vb);
     ALLOC(c->d_p, tb); ALLOC(c->d_force, tb);
     ALLOC(c->d_part_dOd, sizeof(double) * HQMC_MAX_PART); ALLOC(c->d_part_rr, sizeof(double) * HQMC_MAX_PART);
     ALLOC(c->d_part_rz[0], sizeof(double) * HQMC_MAX_PART); ALLOC(c->d_part_rz[1], sizeof(double) * HQMC_MAX_PART);
@@ -168,13 +154,14 @@ extern "C" int hqmc_destroy(hqmc_ctx *c) {
     if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
     if (c->cg_graph) cudaGraphExecDestroy(c->cg_graph);
     if (c->cgb_graph) cudaGraphExecDestroy(c->cgb_graph);
+    for (auto &m : c->md) if (m.exec) cudaGraphExecDestroy(m.exec);
     { void *bp[] = {c->d_cgb_r, c->d_cgb_d, c->d_cgb_Od, c->d_cgb_phi, c->d_cgb_part, c->d_cgb_state, c->d_cgb_ph, c->d_cgb_scal, c->d_cgb_theta0, c->d_cgb_pf}; for (void *p : bp) if (p) cudaFree(p); }
     if (c->h_cgb_state) cudaFreeHost(c->h_cgb_state);
     if (c->h_cgb_scal) cudaFreeHost(c->h_cgb_scal);
     for (auto &ep : c->pending) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (auto &ep : c->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     if (c->ms_plan_ok) cufftDestroy(c->ms_plan);
-    void *ptrs[] = {c->d_ms_a, c->d_ms_b, c->d_ms_acc, c->d_halo, c->d_flags, c->d_r2, c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
+    void *ptrs[] = {c->d_ms_a, c->d_ms_b, c->d_ms_acc, c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
                     c->d_part_rr, c->d_part_rz[0], c->d_part_rz[1], c->d_part_misc, c->d_state, c->d_scal};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (c->h_state) cudaFreeHost(c->h_state);
@@ -283,23 +270,22 @@ extern "C" int hqmc_set_pdl(hqmc_ctx *c, int on) {
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     return HQMC_OK;
 }
-extern "C" int hqmc_set_cg_fusion(hqmc_ctx *c, int on) {
-    if (!c || on < 0 || on > 3) return HQMC_EINVAL;
-    c->cg_defer_x = on == 2 || (on == 0 && cg_defer_default(c));
-    c->fused_allowed = on == 1;
+extern "C" int hqmc_set_md_graph(hqmc_ctx *c, int on) {
+    if (!c) return HQMC_EINVAL;
+    c->md_graph = on != 0;
+    return HQMC_OK;
+}
+extern "C" int hqmc_set_cg_variant(hqmc_ctx *c, int which) {
+    if (!c || which < HQMC_CG_AUTO || which > HQMC_CG_DEFERRED_X) return HQMC_EINVAL;
+    c->cg_defer_x = which == HQMC_CG_DEFERRED_X || (which == HQMC_CG_AUTO && cg_defer_default(c));
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
-    precond_cfg(c, c->pc_kind == 1 ? -c->pc_tile : c->pc_tile);
     return HQMC_OK;
 }
 extern "C" int hqmc_set_mdagm_kernel(hqmc_ctx *c, int which) {
-    if (!c || which < 0 || which > 5) return HQMC_EINVAL;
-    if ((which == 0 && !c->use_stream) || (which == 2 && !c->use_ws) || (which == 3 && !c->use_cluster) || (which >= 4 && !c->use_back))
-        return HQMC_EINVAL;
-    c->stream_on = (which == 0 || which == 2 || which >= 4);
-    c->ws_on = (which == 2);
-    c->back_on = (which >= 4);
-    c->back_coop = (which == 5);
-    c->cluster_on = (which == 3);
+    if (!c || which < HQMC_MDAGM_AUTO || which > HQMC_MDAGM_STREAM) return HQMC_EINVAL;
+    if ((which == HQMC_MDAGM_CLUSTER && !c->use_cluster) || (which == HQMC_MDAGM_STREAM && !c->use_stream)) return HQMC_EINVAL;
+    c->stream_on = which == HQMC_MDAGM_STREAM || (which == HQMC_MDAGM_AUTO && c->use_stream);
+    c->cluster_on = which == HQMC_MDAGM_CLUSTER || (which == HQMC_MDAGM_AUTO && c->use_cluster && !c->use_stream);
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     return hqmc_set_time_tile(c, 0);
 }

@@ -11,11 +11,11 @@
 #include <vector>
 
 #include "../../include/hqmc.h"
+#include "../../include/hqmc_tuning.h"
 #include "cg_kernels.cuh"
 #include "force_kernels.cuh"
 #include "kernels.cuh"
 #include "mdagm_stream.cuh"
-#include "mdagm_ws.cuh"
 #include "mdagm_cluster.cuh"
 #include "mdagm_back.cuh"
 #include "precond_tma.cuh"
@@ -70,14 +70,10 @@ struct hqmc_ctx {
     void *d_ph;          // phase table [Nt][2][L][L] complex
     void *d_packed;      // packed link phases [Nt][4][nb][2] (8 B each) for the streaming M^+M kernel
     double2 *d_tab;      // [2][1024] tanh(a) e^{i k delta} (half step, full step)
-    bool stream_on;      // runtime switch (hqmc_set_mdagm_kernel): a streaming kernel is selected
-    bool use_ws, ws_on;  // warp-specialised strip kernel usable / selected
-    bool back_coop; void *d_halo; unsigned *d_flags;   // halo hand-over between CTAs (k_mdagm_back<COOP>)
-    bool use_back, back_on; size_t back_smem;   // backward-sweep streaming kernel usable / selected
+    bool stream_on;      // runtime switch (hqmc_set_mdagm_kernel): the streaming kernel k_mdagm_back is selected
     bool use_cluster, cluster_on;   // cluster kernel (slice split over R SMs) usable / selected
     int cl_R, cl_threads; size_t cl_smem;
-    size_t ws_smem;
-    bool use_stream;     // streaming kernel usable (BPT == 1 and its shared memory fits)
+    bool use_stream;     // streaming kernel usable (one block per thread and its staging buffers fit one SM)
     size_t stream_smem;
     void *d_r, *d_z, *d_d, *d_Od, *d_X, *d_phi;   // CG vectors, trajectory solution / pseudofermion
     double *d_p, *d_force;                        // host-variant staging
@@ -91,17 +87,13 @@ struct hqmc_ctx {
     int grid_ew, grid_mdagm;
     int pc_tile;         // slices per run of the sliding-window preconditioner kernel (0 = generic kernel)
     int pc_gx, pc_gy, n_part_rz;
-    bool fused_allowed;  // knob (hqmc_set_cg_fusion)
-    bool cg_fused;       // PCG runs on the fused k_cg_rz / k_cg_xd kernels (pc_kind == 2)
-    int f_gx, f_gy, n_part_f; size_t f_smem;
-    void *d_r2;          // second residual buffer (k_cg_rz writes r' out of place)
     int pc_kind;         // 0: generic k_precond, 1: register-ring k_precond_win, 2: TMA-tiled k_precond_tma
     size_t pc_smem;
     // CG chunk graph
     cudaGraphExec_t cg_graph;
     void *cg_graph_x;        // x pointer baked into the graph
     int cg_graph_tile;
-    bool cg_graph_fused, cg_graph_defer;
+    bool cg_graph_defer;
     size_t l2_bytes;     // device L2 size
     // stochastic estimator (hqmc_api_measure.inl): workspace and 3-D FFT plan, created on first use
     bool ms_ready = false, ms_plan_ok = false;
@@ -120,6 +112,16 @@ struct hqmc_ctx {
     int green_batch = 0;                   // hqmc_set_green_batch: 0 = by footprint, 1 = one vector at a time, n = n at a time
     bool cg_defer_x;     // deferred-x PCG vector kernels (k_cg_raxpy + k_cg_xdupdate)
     int cg_chunk;            // iterations per graph launch
+    bool md_graph = true;    // leapfrog steps with fixed-count solves replayed as one CUDA graph (hqmc_set_md_graph)
+    bool md_graph_broken = false;            // capturing a step failed once on this context: plain launches from then on
+    bool capturing_md = false;               // a leapfrog step is being captured (launch() counts into md_nodes_cur)
+    long long cfg_epoch = 0;                 // bumped whenever the PCG chunk graph is rebuilt (kernel selection, taps, tiles, ...)
+    struct MdGraph {                         // [0]: a middle step (closing + opening half kick), [1]: the last step of a trajectory
+        cudaGraphExec_t exec = nullptr;
+        const double *p = nullptr; const void *pf = nullptr; double eps = 0.0; long long iters = -1, epoch = -1;
+        long long nodes[HQMC_K_COUNT] = {};
+    } md[2];
+    long long *md_nodes_cur = nullptr;
     // instrumentation
     bool pdl_next;        // set by a call site whose kernel calls griddepcontrol.wait; consumed by launch()
     int pdl;              // bit per kernel class: programmatic dependent launch of the PCG kernels (hqmc_set_pdl)

@@ -51,22 +51,10 @@ __device__ __forceinline__ void lean_apply_B2(T2 *__restrict__ ex, int nbp, cons
 // grid = G CTAs; CTA i owns slices [i*Nt/G, (i+1)*Nt/G); blockDim.x = nb rounded up to 32.  Arguments as k_mdagm_stream.
 // Slices are addressed by n = t1 - t (n = 0: the halo slice t1 above the run, n = nsl + 1: the halo slice t0 - 1 below);
 // slice n lives in v buffer n mod 3.
-//
-// COOP: no halo recomputation.  The product a = B_{t1-1} v_{t1-1} every CTA forms FIRST is exactly the halo product
-// B_{t0-1} v_{t0-1} its successor (blockIdx + 1) needs in its LAST step: it is published to `halo` (one slice per CTA) and
-// announced through flags[blockIdx] (st.release / ld.acquire at gpu scope; the consumer re-arms the flag).  Every wait is on
-// a LOWER block index, and blocks are dispatched in index order, so the producer is always running or finished: no
-// deadlock whatever the grid size; CTA 0, whose halo belongs to the last CTA, recomputes it as before.
-__device__ __forceinline__ void st_release_gpu(unsigned *p, unsigned v) { asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory"); }
-__device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned *p) {
-    unsigned v; asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
-}
-
-template <typename T, bool DOT, bool COOP>
+template <typename T, bool DOT>
 __global__ void __launch_bounds__(576, 1) k_mdagm_back(Geo g, const typename PhasePack<T>::word *__restrict__ packed,
                         const double2 *__restrict__ tab_g, const typename Cx<T>::type *__restrict__ in,
-                        typename Cx<T>::type *__restrict__ out, T C, double *__restrict__ part, const CgState *__restrict__ st,
-                        typename Cx<T>::type *__restrict__ halo, unsigned *__restrict__ flags) {
+                        typename Cx<T>::type *__restrict__ out, T C, double *__restrict__ part, const CgState *__restrict__ st) {
     typedef typename Cx<T>::type T2;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int nbp = blockDim.x;
@@ -92,8 +80,7 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_back(Geo g, const typename Pha
     auto vb = [&](int n) { return smem_raw + lay.vbuf + (size_t)(n % 3) * vbytes; };
     auto load_v = [&](int n) { bulk_load(vb(n), in_b + (size_t)slice_of(n) * vbytes, vbytes, bar_v + (n % 3)); };
     auto load_p = [&](int n) { bulk_load(pbuf, pk_b + (size_t)slice_of(n) * pbytes, pbytes, bar_p); };
-    const bool consume = COOP && blockIdx.x > 0, produce = COOP && (int)blockIdx.x + 1 < G;
-    const int n_last_v = nsl + 1 - (consume ? 1 : 0);   // last slice index fetched from `in` (the low halo is received instead)
+    const int n_last_v = nsl + 1;                       // last slice index fetched from `in` (the low halo slice t0 - 1)
     uint32_t parv = 0, par_p = 0;                       // bit k of parv: parity of v buffer k
     auto wait_v = [&](int n) { const int k = n % 3; mbar_wait(bar_v + k, (parv >> k) & 1u); parv ^= (1u << k); };
 
@@ -103,7 +90,7 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_back(Geo g, const typename Pha
         if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_TAB * sizeof(double2), bar_t);
         load_p(1);                                      // links of slice t1 - 1: do not depend on the previous kernel
     }
-    pdl_wait();                                         // `in`, `st` and (COOP) the flags are the previous kernels' output
+    pdl_wait();                                         // `in` and `st` are the previous kernels' output
     if (leader) {
         load_v(1); load_v(0);
         if (2 <= n_last_v) load_v(2);
@@ -128,10 +115,6 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_back(Geo g, const typename Pha
     wait_v(1);
     load_block_swz(reinterpret_cast<const T2 *>(vb(1)), b, q0, q1, q2, q3);
     lean_apply_B2(ex, nbp, b, P, q0, q1, q2, q3, []() {}, []() {});
-    if (produce && b.act) {                             // publish B_{t1-1} v_{t1-1} / C for the CTA above: plain stores now,
-        T2 *hb = halo + (size_t)blockIdx.x * g.Vs;      // fence + flag behind the first two barriers of step 0 (off the critical path)
-        hb[b.o0] = q0; hb[b.o1] = q1; hb[b.o2] = q2; hb[b.o3] = q3;
-    }
     {
         const T sC = sC_of(slice_of(1));
         wait_v(0);
@@ -143,45 +126,28 @@ __global__ void __launch_bounds__(576, 1) k_mdagm_back(Geo g, const typename Pha
     for (int j = 0; j < nsl; ++j) {
         const int n = j + 1, t = slice_of(n), tm = slice_of(n + 1);
         const T sCt = sC_of(t), sCm = sC_of(tm);
-        const bool recv = consume && (j == nsl - 1);    // last step: the halo product comes from the CTA below
         if (j == nsl - 1) pdl_launch_dependents();      // let the next kernel's CTAs be dispatched under this CTA's tail
         // 1. q = B_t w_{t+1} / C.  First barrier: everyone is past the previous step -> thread 0 stores out_{t+1} (staged in
         //    buffer n-1) and fetches the links of slice t-1 (pbuf was decoded before the previous step's second sweep).
         //    Second barrier: that store has surely finished reading, so the same buffer can take v_{t-2} (slice n+2).
         lean_apply_B2(ex, nbp, b, P, q0, q1, q2, q3,
             [&]() {
-                if (produce && j == 0) __threadfence();
                 if (leader) {
                     if (j > 0) { bulk_s2g(out_b + (size_t)slice_of(n - 1) * vbytes, vb(n - 1), vbytes); bulk_commit(); }
-                    if (!recv) load_p(n + 1);
+                    load_p(n + 1);
                 }
             },
             [&]() {
-                if (leader) {
-                    if (produce && j == 0) st_release_gpu(flags + blockIdx.x, 1u);
-                    if (n + 2 <= n_last_v) { bulk_wait_read0(); load_v(n + 2); }
-                    if (recv) {                         // buffer (n+1) mod 3 is free: its store finished a step ago
-                        bulk_wait_read0();              // (a store staged in this buffer two steps ago has long been read)
-                        while (ld_acquire_gpu(flags + blockIdx.x - 1) == 0u) { }
-                        asm volatile("fence.proxy.async;" ::: "memory");
-                        bulk_load(vb(n + 1), halo + (size_t)(blockIdx.x - 1) * g.Vs, vbytes, bar_v + ((n + 1) % 3));
-                    }
-                }
+                if (leader && n + 2 <= n_last_v) { bulk_wait_read0(); load_v(n + 2); }
             });
+        // 2. links of slice t-1
+        mbar_wait(bar_p, par_p); par_p ^= 1;
+        lean_load_phases<T>(pbuf, tab, g.nb, qd, P);
+        // 3. a = B_{t-1} v_{t-1} / C
+        wait_v(n + 1);
         T2 a0, a1, a2, a3;
-        if (!recv) {
-            // 2. links of slice t-1
-            mbar_wait(bar_p, par_p); par_p ^= 1;
-            lean_load_phases<T>(pbuf, tab, g.nb, qd, P);
-            // 3. a = B_{t-1} v_{t-1} / C
-            wait_v(n + 1);
-            load_block_swz(reinterpret_cast<const T2 *>(vb(n + 1)), b, a0, a1, a2, a3);
-            lean_apply_B2(ex, nbp, b, P, a0, a1, a2, a3, []() {}, []() {});
-        } else {
-            wait_v(n + 1);
-            load_block_swz(reinterpret_cast<const T2 *>(vb(n + 1)), b, a0, a1, a2, a3);
-            if (leader) st_release_gpu(flags + blockIdx.x - 1, 0u);      // re-arm for the next launch
-        }
+        load_block_swz(reinterpret_cast<const T2 *>(vb(n + 1)), b, a0, a1, a2, a3);
+        lean_apply_B2(ex, nbp, b, P, a0, a1, a2, a3, []() {}, []() {});
         // 4. w_t = v_t - sigma_{t-1} C a;  out_t = w_t - sigma_t C q, staged over v_t;  carry w_t
         T2 *vt = reinterpret_cast<T2 *>(vb(n));
         T2 v0, v1, v2, v3;

@@ -1,4 +1,5 @@
-// mdagm_stream.cuh -- streaming fused O v = M^+ M v kernel (sm_100a): TMA bulk copies + packed link phases.
+// mdagm_stream.cuh -- building blocks of the streaming fused O v = M^+ M v kernels (sm_100a): packed link phases, the lean
+// one-block-per-thread sweep engine, conflict-free staging of slices.  The kernels are in mdagm_back.cuh / mdagm_cluster.cuh.
 //
 //   w_t = v_t - sigma_{t-1} B_{t-1} v_{t-1};   out_t = w_t - sigma_t B_t w_{t+1}      (Eq.8, 284-314)
 //
@@ -207,166 +208,9 @@ __device__ __forceinline__ void store_block_swz(T2 *__restrict__ buf, const Idx 
     buf[sw ? b.o3 : b.o2] = sw ? v3 : v2; buf[sw ? b.o2 : b.o3] = sw ? v2 : v3;
 }
 
-template <typename T> struct StreamSmem {
-    // byte offsets inside dynamic shared memory (nbp = threads per CTA >= nb)
-    size_t tab, vbuf, vbuf2, pbuf, obuf, exch, red, bars, total;
-    __host__ __device__ StreamSmem(int Vs, int nbp) {
-        typedef typename Cx<T>::type T2;
-        size_t o = 0;
-        tab = o;  o += (sizeof(T) == 8) ? (size_t)2 * HQMC_PHASE_TAB * sizeof(double2) : 0;
-        vbuf = o; o += (size_t)Vs * sizeof(T2);
-        vbuf2 = o; o += (size_t)Vs * sizeof(T2);
-        pbuf = o; o += (size_t)2 * Vs * 8;
-        obuf = o; o += (size_t)Vs * sizeof(T2);
-        exch = o; o += (size_t)4 * nbp * sizeof(T2);
-        red = o;  o += 32 * sizeof(double);
-        bars = o; o += 4 * sizeof(uint64_t);
-        total = o;
-    }
-};
-
 __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
     mbar_expect_tx(bar, bytes);
     bulk_g2s(dst, src, bytes, bar);
-}
-
-// ------------------------------------------------------------------------------------------------
-// S5, streaming form.  grid = G CTAs; CTA i owns slices [i*Nt/G, (i+1)*Nt/G); blockDim.x = nb rounded up to 32.
-// packed: [Nt][4][nb][2] PhasePack words;  tab_g: [2][1024] double2 (half step, full step) in global memory.
-// DOT: part[blockIdx] = sum_t ||w_t||^2 over the CTA's slices ( <v, O v> = ||M v||^2 ).
-// Slice bytes must stay below the mbarrier tx-count limit (2^20): checked by the host (use_stream).
-// ------------------------------------------------------------------------------------------------
-template <typename T, bool DOT>
-__global__ void __launch_bounds__(576, 1) k_mdagm_stream(Geo g, const typename PhasePack<T>::word *__restrict__ packed,
-                        const double2 *__restrict__ tab_g, const typename Cx<T>::type *__restrict__ in,
-                        typename Cx<T>::type *__restrict__ out, T C, double *__restrict__ part, const CgState *__restrict__ st) {
-    typedef typename Cx<T>::type T2;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int nbp = blockDim.x;
-    const StreamSmem<T> lay(g.Vs, nbp);
-    const double2 *tab = reinterpret_cast<const double2 *>(smem_raw + lay.tab);
-    unsigned char *pbuf = smem_raw + lay.pbuf;
-    const T2 *vsA = reinterpret_cast<const T2 *>(smem_raw + lay.vbuf), *vsB = reinterpret_cast<const T2 *>(smem_raw + lay.vbuf2);
-    T2 *osm = reinterpret_cast<T2 *>(smem_raw + lay.obuf);
-    T2 *ex = reinterpret_cast<T2 *>(smem_raw + lay.exch);
-    double *red = reinterpret_cast<double *>(smem_raw + lay.red);
-    uint64_t *bar_v = reinterpret_cast<uint64_t *>(smem_raw + lay.bars), *bar_p = bar_v + 1, *bar_t = bar_v + 2, *bar_v2 = bar_v + 3;
-    LeanIdx b;
-    make_lean(g, threadIdx.x, b);
-
-    const int G = gridDim.x;
-    const int t0 = (int)(((long long)blockIdx.x * g.Nt) / G), t1 = (int)(((long long)(blockIdx.x + 1) * g.Nt) / G);
-    if (t0 >= t1) { if (DOT && threadIdx.x == 0) part[blockIdx.x] = 0.0; return; }
-    const uint32_t vbytes = (uint32_t)g.Vs * sizeof(T2), pbytes = (uint32_t)g.Vs * 16;
-    const unsigned char *in_b = reinterpret_cast<const unsigned char *>(in);
-    const unsigned char *pk_b = reinterpret_cast<const unsigned char *>(packed);
-    unsigned char *out_b = reinterpret_cast<unsigned char *>(out);
-    const bool leader = threadIdx.x == 0;
-    uint32_t par_vA = 0, par_vB = 0, par_p = 0;
-    const int tp = (t0 == 0) ? g.Nt - 1 : t0 - 1;
-    const int nsl = t1 - t0;
-    auto wrap = [&](int t) { return t >= g.Nt ? t - g.Nt : t; };
-
-    // v is kept TWO slices deep (buffers A, B alternate), the links one slice deep: every copy is issued a full
-    // slice of compute before it is needed, so HBM stays busy while the sweeps run.
-    if (leader) {
-        mbar_init(bar_v, 1); mbar_init(bar_v2, 1); mbar_init(bar_p, 1); mbar_init(bar_t, 1);
-        mbar_fence_init();
-        if (sizeof(T) == 8) bulk_load(smem_raw + lay.tab, tab_g, 2 * HQMC_PHASE_TAB * sizeof(double2), bar_t);
-        bulk_load(smem_raw + lay.vbuf, in_b + (size_t)tp * vbytes, vbytes, bar_v);
-        bulk_load(pbuf, pk_b + (size_t)tp * pbytes, pbytes, bar_p);
-        bulk_load(smem_raw + lay.vbuf2, in_b + (size_t)t0 * vbytes, vbytes, bar_v2);
-    }
-    // The CG "done" flag is read only now, with the first slices already in flight (its latency is hidden).
-    const int done = (st != nullptr) ? *(volatile const int *)&st->done : 0;
-    __syncthreads();                      // barrier inits visible to every thread
-    if (sizeof(T) == 8) mbar_wait(bar_t, 0);
-    if (done) {                           // drain the copies aimed at this CTA's shared memory, then leave
-        mbar_wait(bar_v, 0); mbar_wait(bar_v2, 0); mbar_wait(bar_p, 0);
-        return;
-    }
-
-    T2 w0, w1, w2, w3;                    // w_t
-    LeanPh<T2> P;
-    double acc = 0.0;
-
-    // ---- prologue: w_{t0} = v_{t0} - sigma_{tp} C B_{tp} v_{tp}
-    mbar_wait(bar_v, par_vA); par_vA ^= 1;
-    mbar_wait(bar_p, par_p); par_p ^= 1;
-    load_block_swz(vsA, b, w0, w1, w2, w3);
-    lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
-    lean_apply_B(ex, nbp, b, P, w0, w1, w2, w3, [&]() {
-        if (leader) {                     // buffer A and pbuf have been read by everyone
-            bulk_load(smem_raw + lay.vbuf, in_b + (size_t)wrap(t0 + 1) * vbytes, vbytes, bar_v);
-            bulk_load(pbuf, pk_b + (size_t)t0 * pbytes, pbytes, bar_p);
-        }
-    });
-    {
-        const T sC = (tp == g.Nt - 1) ? C : -C;
-        mbar_wait(bar_v2, par_vB); par_vB ^= 1;
-        mbar_wait(bar_p, par_p); par_p ^= 1;
-        T2 v0, v1, v2, v3;
-        load_block_swz(vsB, b, v0, v1, v2, v3);
-        w0.x = fma(sC, w0.x, v0.x); w0.y = fma(sC, w0.y, v0.y); w1.x = fma(sC, w1.x, v1.x); w1.y = fma(sC, w1.y, v1.y);
-        w2.x = fma(sC, w2.x, v2.x); w2.y = fma(sC, w2.y, v2.y); w3.x = fma(sC, w3.x, v3.x); w3.y = fma(sC, w3.y, v3.y);
-        lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
-    }
-
-    for (int i = 0; i < nsl; ++i) {
-        const int t = t0 + i;
-        const int tn = wrap(t + 1);
-        const T sC = (t == g.Nt - 1) ? C : -C;
-        const bool more = (i + 1 < nsl);
-        const bool odd = i & 1;
-        const T2 *vcur = odd ? vsA : vsB, *vnxt = odd ? vsB : vsA;       // v_t sits in buffer (i+1)&1, v_{t+1} in buffer i&1
-        // v = B_t v_t / C.  After the first barrier of the sweep sequence everyone has read v_t and (at the end of the
-        // previous iteration) the links, and obuf holds out_{t-1} completely: thread 0 stores it and fetches v_{t+2}
-        // into the buffer v_t occupied and the links of slice t+1.
-        T2 v0, v1, v2, v3;
-        load_block_swz(vcur, b, v0, v1, v2, v3);
-        lean_apply_B(ex, nbp, b, P, v0, v1, v2, v3, [&]() {
-            if (leader) {
-                if (i > 0) { bulk_s2g(out_b + (size_t)(t - 1) * vbytes, osm, vbytes); bulk_commit(); }
-                if (more) {
-                    bulk_load(smem_raw + (odd ? lay.vbuf : lay.vbuf2), in_b + (size_t)wrap(t + 2) * vbytes, vbytes, odd ? bar_v : bar_v2);
-                    bulk_load(pbuf, pk_b + (size_t)tn * pbytes, pbytes, bar_p);
-                }
-            }
-        });
-        if (odd) { mbar_wait(bar_v2, par_vB); par_vB ^= 1; } else { mbar_wait(bar_v, par_vA); par_vA ^= 1; }
-        T2 n0, n1, n2, n3;                                                         // v_{t+1}
-        load_block_swz(vnxt, b, n0, n1, n2, n3);
-        T2 q0, q1, q2, q3;                                                         // w_{t+1}, then B_t w_{t+1}
-        q0.x = fma(sC, v0.x, n0.x); q0.y = fma(sC, v0.y, n0.y); q1.x = fma(sC, v1.x, n1.x); q1.y = fma(sC, v1.y, n1.y);
-        q2.x = fma(sC, v2.x, n2.x); q2.y = fma(sC, v2.y, n2.y); q3.x = fma(sC, v3.x, n3.x); q3.y = fma(sC, v3.y, n3.y);
-        const T2 k0 = q0, k1 = q1, k2 = q2, k3 = q3;                               // keep w_{t+1}
-        // The store of out_{t-1} must have finished READING obuf before obuf is rewritten below: thread 0 waits
-        // for that before the first barrier of this sweep sequence.
-        if (leader) bulk_wait_read0();
-        lean_apply_B(ex, nbp, b, P, q0, q1, q2, q3, []() {});
-        if (DOT && b.act)
-            acc += ((double)w0.x * w0.x + (double)w0.y * w0.y) + ((double)w1.x * w1.x + (double)w1.y * w1.y) +
-                   ((double)w2.x * w2.x + (double)w2.y * w2.y) + ((double)w3.x * w3.x + (double)w3.y * w3.y);
-        q0.x = fma(sC, q0.x, w0.x); q0.y = fma(sC, q0.y, w0.y); q1.x = fma(sC, q1.x, w1.x); q1.y = fma(sC, q1.y, w1.y);
-        q2.x = fma(sC, q2.x, w2.x); q2.y = fma(sC, q2.y, w2.y); q3.x = fma(sC, q3.x, w3.x); q3.y = fma(sC, q3.y, w3.y);
-        w0 = k0; w1 = k1; w2 = k2; w3 = k3;
-        if (b.act) store_block_swz(osm, b, q0, q1, q2, q3);
-        fence_async_smem();               // my obuf writes -> visible to the async proxy (the store is issued after the next barrier)
-        if (more) {
-            mbar_wait(bar_p, par_p); par_p ^= 1;
-            lean_load_phases<T>(pbuf, tab, g.nb, b.act ? b.q : 0, P);
-        }
-    }
-    __syncthreads();
-    if (leader) {
-        bulk_s2g(out_b + (size_t)(t1 - 1) * vbytes, osm, vbytes);
-        bulk_commit();
-        bulk_wait0();
-    }
-    if (DOT) {
-        double s = block_sum(acc, red);
-        if (threadIdx.x == 0) part[blockIdx.x] = s;
-    }
 }
 
 }  // namespace hqmc

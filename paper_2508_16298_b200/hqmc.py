@@ -17,16 +17,18 @@ LIB_PATH = os.path.join(_HERE, "libhqmc.so")
 
 HQMC_OK, HQMC_EINVAL, HQMC_ECUDA, HQMC_ENOCONV, HQMC_ENOMEM = 0, -1, -2, -3, -4
 K_MDAGM, K_AXPY, K_PRECOND, K_DUPDATE, K_M, K_FORCE, K_PHASE, K_MISC, K_COUNT = range(9)
+MDAGM_AUTO, MDAGM_REGISTER, MDAGM_CLUSTER, MDAGM_STREAM = 0, 1, 2, 3
+CG_AUTO, CG_TEXTBOOK, CG_DEFERRED_X = 0, 1, 2
 KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force", "phase", "misc"]
 
-# every symbol include/hqmc.h declares
+# every symbol include/hqmc.h and include/hqmc_tuning.h declare
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
     "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
-    "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_fusion", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
+    "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_variant", "hqmc_set_md_graph", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
 
 
@@ -121,14 +123,18 @@ class HQMC:
         _check(_lib.hqmc_set_time_tile(self._ctx, C.c_int(tt)))
 
     def set_mdagm_kernel(self, which: int):
-        """0 = streaming (TMA) kernel, 1 = register-only kernel."""
+        """MDAGM_AUTO / MDAGM_REGISTER / MDAGM_CLUSTER / MDAGM_STREAM (include/hqmc_tuning.h)."""
         _check(_lib.hqmc_set_mdagm_kernel(self._ctx, C.c_int(which)))
 
     def set_precond_tile(self, slices_per_run: int):
         _check(_lib.hqmc_set_precond_tile(self._ctx, C.c_int(slices_per_run)))
 
-    def set_cg_fusion(self, on: int):
-        _check(_lib.hqmc_set_cg_fusion(self._ctx, C.c_int(int(on))))
+    def set_cg_variant(self, which: int):
+        """CG_AUTO / CG_TEXTBOOK / CG_DEFERRED_X (include/hqmc_tuning.h)."""
+        _check(_lib.hqmc_set_cg_variant(self._ctx, C.c_int(int(which))))
+
+    def set_md_graph(self, on: bool):
+        _check(_lib.hqmc_set_md_graph(self._ctx, C.c_int(int(on))))
 
     def set_pdl(self, on: int):
         _check(_lib.hqmc_set_pdl(self._ctx, C.c_int(int(on))))

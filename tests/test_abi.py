@@ -1,4 +1,4 @@
-"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/hqmc.h declares, validates
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/*.h declares, validates
 arguments, and fails loudly (no CPU fallback) when there is no CUDA device."""
 import ctypes as C
 import os
@@ -11,9 +11,18 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared():
-    txt = open(os.path.join(ROOT, "include", "hqmc.h")).read()
-    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    return sorted(set(re.findall(r"\b(hqmc_[a-z_A-Z0-9]+)\s*\(", txt)))
+    names = set()
+    for h in ("hqmc.h", "hqmc_tuning.h"):
+        txt = open(os.path.join(ROOT, "include", h)).read()
+        txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+        names |= set(re.findall(r"\b(hqmc_[a-z_A-Z0-9]+)\s*\(", txt))
+    return sorted(names)
+
+
+def test_hot_path_header_has_no_tuning_knobs():
+    """include/hqmc.h lists the operations of the method, their batched / estimator / host forms and nothing else."""
+    txt = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "hqmc.h")).read(), flags=re.S)
+    assert not re.findall(r"\bhqmc_(set_(?!precond|theta)[a-z_]+|reset_stats|get_kernel_stats)\s*\(", txt)
 
 
 def test_library_loads_and_exports_every_declared_symbol():
