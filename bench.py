@@ -35,9 +35,6 @@ METRIC = "MdagM_Gsite_per_s"
 UNIT = "Gsite/s"
 # algorithmic bytes per site (complex128): read v (16) + 2 link phases as theta (16) + write (16)
 BYTES_PER_SITE = {"mdagm": 48.0, "cg_axpy": 96.0, "precond": 32.0, "cg_dupdate": 48.0}
-# fused PCG vector kernels (default): "precond" class = k_cg_rz (read r, Od; write r', z), "cg_dupdate" class = k_cg_xd
-# (read x, d, z; write x, d)
-BYTES_PER_SITE_FUSED = {"mdagm": 48.0, "precond": 64.0, "cg_dupdate": 80.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/), L=48, c128
 TRAFFIC_NCU = {"mdagm": 35.5e6}
 
@@ -140,12 +137,12 @@ def run_reference(args):
             times.append(dt); apps += a
     total = sum(times)
     value = apps * N / total / 1e9
-    sample = (f"same lattice (L={L}, Ntau={Ntau}), same step structure, fixed-count CG cut to {iters} iterations per solve "
-              f"({2 * iters} M^+M per step) instead of {args.cg_iters}")
+    sample = (f"bounded sample of the workload: same lattice (L={L}, Ntau={Ntau}), same step structure, each fixed-count solve cut to "
+              f"{iters} of its {args.cg_iters} PCG iterations ({2 * iters} M^+M per step); the metric is per M^+M application")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total / max(1, len(times)), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(args, L, Ntau, iters),
+            "config": workload_config(args, L, Ntau, args.cg_iters),     # the workload; `sample` says what was run of it
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -275,8 +272,7 @@ def run_gpu(args):
     value = total_apps * N / (ms * 1e-3) / 1e9
     e2e_value = total_e2e_apps * N / e2e_s / 1e9
     peak, peak_src = measured_peaks()
-    fused = "cg_axpy" not in kern["us"]
-    bps = dict(BYTES_PER_SITE_FUSED if fused else BYTES_PER_SITE)
+    bps = dict(BYTES_PER_SITE)
     if prec != "c128":
         bps = {k: v / 2 for k, v in bps.items()}
     per_kernel = {}
@@ -286,7 +282,8 @@ def run_gpu(args):
     dom = max(per_kernel, key=lambda k: per_kernel[k]["us_in_graph"])
     achieved = per_kernel[dom]["alg_GBps"]
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": TRAFFIC_NCU.get(dom), "peak_source": peak_src, "alg_bytes_per_site": bps[dom],
+                "traffic": TRAFFIC_NCU.get(dom), "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of the committed ncu --set full capture (profiles/r02_summary.md); not measured by this run",
+                "peak_source": peak_src, "alg_bytes_per_site": bps[dom],
                 "how": "leave-one-out CUDA-event timing of the graph-replayed fixed-count PCG solve (bench.py pcg_kernel_costs)"}
     # the whole PCG iteration against the same peak: algorithmic bytes of all its kernels / the iteration time.  The vector
     # kernels are served largely from L2 (their alg_GBps can exceed the HBM peak), so this is a figure of merit against the
@@ -308,7 +305,15 @@ def run_gpu(args):
                                        f"({cb_apps} M^+M), {cb_dt:.1f} s"},
             "cg_us_per_iter": us_per_iter, "cg_iters_per_s": 1e6 / us_per_iter, "cg_ms_per_solve_fixed": us_per_iter * I * 1e-3,
             "ms_per_trajectory_step": ms_per_step, "kernels": per_kernel, "mdagm_sweep": sweep,
-            "dH": r["H1"] - r["H0"]}
+            # BASELINE's first figure, for the M^+M kernel itself (`value` charges the whole step to the M^+M count)
+            "mdagm_kernel": {"us_in_graph": per_kernel["mdagm"]["us_in_graph"], "Gsite_per_s": N / per_kernel["mdagm"]["us_in_graph"] / 1e3,
+                             "alg_GBps": per_kernel["mdagm"]["alg_GBps"], "frac_of_peak": per_kernel["mdagm"]["alg_GBps"] / peak},
+            "dH_fixed_count_unconverged": r["H1"] - r["H0"]}
+    if world == 1 and not args.no_extras:
+        try:
+            line.update(contract_numbers(args, torch, hqmc, inputs, theta0, inputs.complex_gaussian((Ntau, L, L), seed)))
+        except Exception as e:                                           # never lose the metric line over the extra keys
+            line["contract_numbers_error"] = repr(e)[:300]
     if world == 1 and not args.no_small:
         line["batched_chains"] = small_lattice_chains(torch, hqmc, inputs, args.cg_iters)
     print(json.dumps(line))
@@ -316,6 +321,109 @@ def run_gpu(args):
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def contract_numbers(args, torch, hqmc, inputs, theta_cfg, eta_cfg):
+    """The figures BASELINE.json's metric and configs name beyond the timed step, measured in the same run (rank 0, N = 1):
+    `cg_solve`  -- config 4's "preconditioned CG to 1e-10, with iteration count and ms per solve": on BASELINE's uniform field
+                   and on a paper-regime field (c_tau = 80, K = 1), with the recurrence residual and the residual of the
+                   GPU solution under the ORACLE's operator (one CPU M^+M after the timed region; reading C16 i);
+    `c64`       -- the complex64 variant "timed separately": M^+M and PCG iteration in the replayed graph;
+    `config5`   -- L=64, Ntau=640 on its seeded heat-bath field: ms per 20-step trajectory (fixed-count protocol), M^+M us;
+    `md_graph`  -- leapfrog step replayed as one CUDA graph against plain launches (the paper reports
+                   2-5 x from CUDA graphs for L < 30 and 1-2 x above, on its GPU, for whole sweeps) at L = 12, 24, 48."""
+    from oracle import oracle as orc
+    out = {}
+    c = inputs.CONFIGS[args.config]
+    L, Ntau, N = c["L"], c["Ntau"], c["L"] * c["L"] * c["Ntau"]
+    orc.build(); orc.set_threads(max(orc.max_threads(), len(os.sched_getaffinity(0))))
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    def solve_on(theta, label, **kw):
+        g = hqmc.HQMC(L, Ntau, **kw)
+        g.set_theta(dev(theta))
+        phi = g.apply_Mdag(dev(eta_cfg))
+        x = g.new_vec()
+        g.cg_solve(phi, 0.0, 64, x=x)                               # graph capture outside the timed solve
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); x, it, rel, ok = g.cg_solve(phi, args.tol, args.max_iter, x=x); e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        phi_h, x_h = phi.cpu().numpy(), x.cpu().numpy()
+        o = orc.Oracle(L, Ntau, **kw)
+        res_orc = float(np.linalg.norm((phi_h - o.apply_MdagM(theta, x_h)).ravel()) / np.linalg.norm(phi_h.ravel()))
+        g.close()
+        return {"field": label, "tol": args.tol, "iterations": it, "converged": bool(ok), "ms_per_solve": ms, "us_per_iter": 1e3 * ms / max(1, it),
+                "recurrence_relres": rel, "oracle_operator_relres": res_orc}
+
+    if not args.no_solve:
+        out["cg_solve"] = {
+            "baseline_field": solve_on(theta_cfg, "BASELINE config 4: theta uniform[-pi,pi)"),
+            "paper_regime_field": solve_on(inputs.theta_paper_regime(L, Ntau, c["seed"], sweeps=20),
+                                           "paper regime: heat bath at c_tau = 1/(J dtau^2) = 80, K = 1 (PAPER.md:107), cold start, 20 sweeps",
+                                           c_tau=80.0, K=1.0)}
+    # complex64 variant (BASELINE config 4: "with a complex64 variant timed separately")
+    g = hqmc.HQMC(L, Ntau, prec="c64")
+    g.set_theta(dev(theta_cfg))
+    phi = g.apply_Mdag(dev(eta_cfg.astype(np.complex64)))
+    k64 = pcg_kernel_costs(g, torch, phi, args.cg_iters)
+    out["c64"] = {"mdagm_us_in_graph": k64["us"]["mdagm"], "mdagm_Gsite_per_s": N / k64["us"]["mdagm"] / 1e3,
+                  "mdagm_alg_GBps": 24.0 * N / k64["us"]["mdagm"] / 1e3, "cg_us_per_iter": k64["iter_us"], "kernels_us": k64["us"]}
+    g.close()
+    # config 5 on its own field
+    if not args.no_config5:
+        c5 = inputs.CONFIGS[5]
+        L5, Nt5, N5 = c5["L"], c5["Ntau"], c5["L"] * c5["L"] * c5["Ntau"]
+        th5 = inputs.make_theta(5)
+        g = hqmc.HQMC(L5, Nt5)
+        d_th0 = dev(th5)
+        g.set_theta(d_th0)
+        phi = g.apply_Mdag(dev(inputs.complex_gaussian((Nt5, L5, L5), c5["seed"])))
+        k5 = pcg_kernel_costs(g, torch, phi, args.cg_iters)
+        ms = []
+        for k in range(2):                                          # first trajectory is warm-up
+            d_th, d_p = d_th0.clone(), dev(inputs.momenta(L5, Nt5, c5["seed"] + k))
+            g.set_theta(d_th)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); r = g.trajectory(d_th, d_p, phi, 20, 0.05, cg_tol=0.0, cg_max_iter=args.cg_iters); e1.record(); torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        peak, _ = measured_peaks()
+        out["config5"] = {"L": L5, "Ntau": Nt5, "sites": N5, "theta": "seeded heat bath at 1/g^2 = 1 + pi flux (BASELINE config 5)",
+                          "protocol": f"20 leapfrog steps, eps 0.05, {args.cg_iters} fixed PCG iterations per solve (PAPER.md:348), 21 solves",
+                          "ms_per_trajectory": ms[1], "cg_iters_per_trajectory": r["cg_iters"], "us_per_cg_iter_all_in": 1e3 * ms[1] / r["cg_iters"],
+                          "MdagM_Gsite_per_s_all_in": r["cg_iters"] * N5 / (ms[1] * 1e-3) / 1e9,
+                          "hbm_fraction_alg": 224.0 * N5 * r["cg_iters"] / (ms[1] * 1e-3) / 1e9 / peak,
+                          "mdagm_us_in_graph": k5["us"]["mdagm"], "mdagm_Gsite_per_s": N5 / k5["us"]["mdagm"] / 1e3,
+                          "mdagm_alg_GBps": 48.0 * N5 / k5["us"]["mdagm"] / 1e3, "cg_us_per_iter": k5["iter_us"], "kernels_us": k5["us"]}
+        g.close()
+    # leapfrog step as one CUDA graph vs plain launches
+    mg = {"protocol": "3 leapfrog steps, eps 0.01, 100 fixed PCG iterations per solve, uniform theta; ms per trajectory, best of 5",
+          "paper": "PAPER.md:334-350: CUDA graphs give 2-5 x for L < 30 and 1-2 x for larger lattices (its GPU, whole sweeps) -- context"}
+    for Lg in (12, 24, 48):
+        Ng = 10 * Lg
+        th, p0 = inputs.theta_uniform(Lg, Ng, 7), inputs.momenta(Lg, Ng, 7)
+        res, fin = {}, {}
+        for on in (True, False):
+            g = hqmc.HQMC(Lg, Ng)
+            g.set_md_graph(on)
+            g.set_theta(dev(th))
+            phi = g.apply_Mdag(dev(inputs.complex_gaussian((Ng, Lg, Lg), 7)))
+            best = 1e30
+            for k in range(6):
+                d_th, d_p = dev(th), dev(p0)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); g.trajectory(d_th, d_p, phi, 3, 0.01, cg_tol=0.0, cg_max_iter=100); e1.record(); torch.cuda.synchronize()
+                if k:
+                    best = min(best, e0.elapsed_time(e1))
+            res["graph" if on else "plain"] = best
+            fin[on] = (d_th, d_p)
+            g.close()
+        mg[f"L{Lg}"] = {"ms_graph": res["graph"], "ms_plain": res["plain"], "speedup": res["plain"] / res["graph"],
+                        "bitwise_identical": bool(torch.equal(fin[True][0], fin[False][0]) and torch.equal(fin[True][1], fin[False][1]))}
+    out["md_graph"] = mg
+    return out
 
 
 def small_lattice_chains(torch, hqmc, inputs, cg_iters, L=16, n_chain=40, md_steps=3, eps=0.01):
@@ -372,7 +480,7 @@ def pcg_kernel_costs(g, torch, d_phi, iters):
     full = run()
     g.reset_stats(); g.cg_solve(d_phi, 0.0, 32, x=x); torch.cuda.synchronize()
     used = [k for k in ("mdagm", "cg_axpy", "precond", "cg_dupdate") if g.kernel_stats()[k][0] >= 32]
-    keeper = "cg_dupdate" if "cg_axpy" not in used else "precond"     # the class that counts iterations / sets `done`
+    keeper = "precond"                                                # the class that counts iterations / sets `done`
     out = {}
     for k in used:
         if k == keeper:
@@ -590,6 +698,9 @@ def main():
     ap.add_argument("--prec", default="c128", choices=["c128", "c64"])
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-small", action="store_true", help="skip the extra small-lattice batched-chains key of the JSON line")
+    ap.add_argument("--no-extras", action="store_true", help="skip cg_solve / c64 / config5 / md_graph keys (converged solves, second lattice)")
+    ap.add_argument("--no-solve", action="store_true", help="skip the converged config-4 solves (about 20 s of GPU time)")
+    ap.add_argument("--no-config5", action="store_true", help="skip the L=64 lattice (its heat-bath field costs 40 s of host time)")
     ap.add_argument("--mode", default="step", choices=["step", "solve", "measure", "trajectory"],
                     help="solve: one full PCG solve to --tol; measure: the stochastic estimator on a paper-regime field (neither is the timed metric)")
     ap.add_argument("--n-traj", type=int, default=5, help="trajectory mode: timed trajectories (BASELINE config 5: 5)")

@@ -416,3 +416,72 @@ int orc_hqmc_step(const orc_params *P, double *theta, double *p, const cplx *eta
     free(phi); free(theta0);
     return accepted;
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * Random numbers of the HQMC update (PAPER.md:185 step (i): "sample p and R from Gaussian distributions"
+ * step (iii): uniform u; reading C6: weights e^{-R^+R} and e^{-sum p^2}, so Re R, Im R, p ~ N(0, 1/2), E|R|^2 = 1).
+ * The paper names no generator.  Both sides implement the SAME counter-based one, so that a sweep is reproducible from
+ * (seed, update index) alone: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11: ten rounds of
+ *     (c0, c1, c2, c3) <- (hi(M1 c2) ^ c1 ^ k0, lo(M1 c2), hi(M0 c0) ^ c3 ^ k1, lo(M0 c0)),  then (k0, k1) += (W0, W1)
+ * with M0 = 0xD2511F53, M1 = 0xCD9E8D57, W0 = 0x9E3779B9, W1 = 0xBB67AE85), counter = (index lo, index hi, stream, update),
+ * key = (seed lo, seed hi); streams: 0 = R (eta), 1 = p, 2 = Metropolis u.  From the four output words x0..x3:
+ *     u1 = ((x0 >> 5) 2^26 + (x1 >> 6)) / 2^53,   u2 = ((x2 >> 5) 2^26 + (x3 >> 6)) / 2^53      (both in [0, 1))
+ * and by Box-Muller the pair  sqrt(-ln(1 - u1)) (cos 2 pi u2, sin 2 pi u2): two independent N(0, 1/2).
+ * Element i of stream 0 is the complex number R_i; element i of stream 1 is the pair (p_{2i}, p_{2i+1}).
+ * Pins (tests/test_oracle_rng.py): the published known-answer vectors of Philox4x32-10; moments and a Kolmogorov-Smirnov
+ * bound of the uniforms and Gaussians; E|R|^2 = 1, Var p = 1/2.
+ * ------------------------------------------------------------------------------------------- */
+#include <stdint.h>
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+static void rng_words(uint64_t seed, uint32_t update, uint32_t stream, uint64_t i, uint32_t x[4]) {
+    const uint32_t ctr[4] = {(uint32_t)i, (uint32_t)(i >> 32), stream, update}, key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    orc_philox4x32_10(ctr, key, x);
+}
+/* raw words of elements 0..n-1: out[4 n] */
+void orc_rng_raw(uint64_t seed, uint32_t update, uint32_t stream, long n, uint32_t *out) {
+    for (long i = 0; i < n; ++i) rng_words(seed, update, stream, (uint64_t)i, out + 4 * i);
+}
+static double u53(uint32_t a, uint32_t b) { return ((double)(a >> 5) * 67108864.0 + (double)(b >> 6)) * (1.0 / 9007199254740992.0); }
+/* the two uniforms of elements 0..n-1: out[2 n] */
+void orc_rng_uniform(uint64_t seed, uint32_t update, uint32_t stream, long n, double *out) {
+    for (long i = 0; i < n; ++i) {
+        uint32_t x[4];
+        rng_words(seed, update, stream, (uint64_t)i, x);
+        out[2 * i] = u53(x[0], x[1]); out[2 * i + 1] = u53(x[2], x[3]);
+    }
+}
+/* the Gaussian pair (variance 1/2 each) of elements 0..n-1: out[2 n] */
+void orc_rng_gauss(uint64_t seed, uint32_t update, uint32_t stream, long n, double *out) {
+    for (long i = 0; i < n; ++i) {
+        uint32_t x[4];
+        rng_words(seed, update, stream, (uint64_t)i, x);
+        const double u1 = u53(x[0], x[1]), u2 = u53(x[2], x[3]);
+        const double r = sqrt(-log(1.0 - u1)), a = 6.283185307179586476925286766559 * u2;
+        out[2 * i] = r * cos(a); out[2 * i + 1] = r * sin(a);
+    }
+}
+/* `n_updates` HQMC updates (steps (i)-(iv)) from update index `first`: update k draws R from stream 0,
+ * p from stream 1 and u = first uniform of element 0 of stream 2, all at counter word `update` = k.  Per-update outputs. */
+void orc_hqmc_sweep(const orc_params *P, double *theta, uint64_t seed, uint32_t first, int n_updates, int nsteps, double eps,
+                    double cg_tol, long cg_max_iter, double *H0, double *H1, int *accepted, long *iters) {
+    const size_t N = (size_t)P->Ntau * P->L * P->L;
+    cplx *eta = (cplx *)malloc(sizeof(cplx) * N);
+    double *p = (double *)malloc(sizeof(double) * 2 * N), u2[2];
+    for (int k = 0; k < n_updates; ++k) {
+        const uint32_t upd = first + (uint32_t)k;
+        orc_rng_gauss(seed, upd, 0, (long)N, (double *)eta);
+        orc_rng_gauss(seed, upd, 1, (long)N, p);
+        orc_rng_uniform(seed, upd, 2, 1, u2);
+        accepted[k] = orc_hqmc_step(P, theta, p, eta, u2[0], nsteps, eps, cg_tol, cg_max_iter, H0 + k, H1 + k, iters + k);
+    }
+    free(eta); free(p);
+}

@@ -69,6 +69,33 @@ def get_threads() -> int:
     return int(lib().orc_get_threads())
 
 
+def philox4x32_10(ctr, key):
+    """One block of the counter-based generator both sides use (hqmc_oracle.c): 4 counter words, 2 key words -> 4 words."""
+    c = (C.c_uint32 * 4)(*[int(x) & 0xFFFFFFFF for x in ctr]); k = (C.c_uint32 * 2)(*[int(x) & 0xFFFFFFFF for x in key])
+    out = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, out)
+    return [int(x) for x in out]
+
+
+def rng_raw(seed: int, update: int, stream: int, n: int) -> np.ndarray:
+    out = np.empty(4 * n, dtype=np.uint32)
+    lib().orc_rng_raw(C.c_uint64(seed), C.c_uint32(update), C.c_uint32(stream), C.c_long(n), out.ctypes.data_as(C.c_void_p))
+    return out.reshape(n, 4)
+
+
+def rng_uniform(seed: int, update: int, stream: int, n: int) -> np.ndarray:
+    out = np.empty(2 * n)
+    lib().orc_rng_uniform(C.c_uint64(seed), C.c_uint32(update), C.c_uint32(stream), C.c_long(n), out.ctypes.data_as(C.c_void_p))
+    return out.reshape(n, 2)
+
+
+def rng_gauss(seed: int, update: int, stream: int, n: int) -> np.ndarray:
+    """n pairs of independent N(0, 1/2) (reading C6): stream 0 = R as (re, im), stream 1 = p in pairs."""
+    out = np.empty(2 * n)
+    lib().orc_rng_gauss(C.c_uint64(seed), C.c_uint32(update), C.c_uint32(stream), C.c_long(n), out.ctypes.data_as(C.c_void_p))
+    return out.reshape(n, 2)
+
+
 def precond_taps(L: int, dtau: float = 0.1, t: float = 1.0, W: int = 6):
     """(c_0..c_W, p_0..p_W) of reading C10, from the oracle's own B at pi-flux."""
     c = np.zeros(W + 1)
@@ -190,3 +217,16 @@ class Oracle:
                                   C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_long(cg_max_iter), C.byref(H0),
                                   C.byref(H1), C.byref(it))
         return dict(theta=th, p=pp, H0=H0.value, H1=H1.value, accepted=bool(acc), cg_iters=int(it.value))
+
+    def hqmc_sweep(self, theta, seed: int, first: int, n_updates: int, nsteps: int, eps: float, cg_tol: float = 1e-13,
+                   cg_max_iter: int = 1000000):
+        """n_updates HQMC updates with the oracle's own counter-based draws -> dict(theta, H0, H1, accepted,
+        cg_iters), one entry per update.  theta is not modified."""
+        th = np.array(theta, dtype=np.float64, order="C").copy()
+        H0, H1 = np.zeros(n_updates), np.zeros(n_updates)
+        acc, it = np.zeros(n_updates, dtype=np.int32), np.zeros(n_updates, dtype=np.int64)
+        lib().orc_hqmc_sweep(self._p, th.ctypes.data_as(C.c_void_p), C.c_uint64(seed), C.c_uint32(first), C.c_int(n_updates),
+                             C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_long(cg_max_iter),
+                             H0.ctypes.data_as(C.c_void_p), H1.ctypes.data_as(C.c_void_p), acc.ctypes.data_as(C.c_void_p),
+                             it.ctypes.data_as(C.c_void_p))
+        return dict(theta=th, H0=H0, H1=H1, accepted=acc.astype(bool), cg_iters=it)

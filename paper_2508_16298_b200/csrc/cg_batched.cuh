@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(128) k_cgb_precond(Geo g, Taps taps, const typ
             } else {
                 long long it = st->iters + 1;
                 st->iters = it; st->rr = rr;
-                if ((st->tol2 > 0.0 && rr <= st->tol2 * st->bb) || it >= st->max_iter || rr != rr) st->done = 1;   // a non-finite residual stops the solve
+                if ((st->tol2 > 0.0 && (rr <= st->tol2 * st->bb || rr != rr)) || it >= st->max_iter) st->done = 1;   // a non-finite residual ends a tolerance-stopped solve (a fixed-count one runs its count)
             }
         }
     }
@@ -175,7 +175,7 @@ __global__ void k_cgb_precond_gen(Geo g, Taps taps, const typename Cx<T>::type *
             } else {
                 long long it = st->iters + 1;
                 st->iters = it; st->rr = rr;
-                if ((st->tol2 > 0.0 && rr <= st->tol2 * st->bb) || it >= st->max_iter || rr != rr) st->done = 1;   // a non-finite residual stops the solve
+                if ((st->tol2 > 0.0 && (rr <= st->tol2 * st->bb || rr != rr)) || it >= st->max_iter) st->done = 1;   // a non-finite residual ends a tolerance-stopped solve (a fixed-count one runs its count)
             }
         }
     }
