@@ -145,6 +145,24 @@ int hqmc_hqmc_step(hqmc_ctx *ctx, double *d_theta, double *d_p, const void *d_et
                    double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out, int *accepted_out,
                    long long *cg_iters_out);
 
+/* Random numbers of the update, drawn on the device (PAPER.md:185 step (i), :199 step (iii); readings C6, C25).  Counter
+ * based: element i of stream s of update k is the Philox4x32-10 block at counter (i lo, i hi, s, k) under key (seed lo,
+ * seed hi); streams 0 = R, 1 = p, 2 = u; two 53-bit uniforms per block, Box-Muller pair sqrt(-ln(1 - u1)) (cos, sin)(2 pi u2):
+ * two independent N(0, 1/2).  hqmc_rng_raw: the four words of elements 0..n-1 (d_out[4 n], uint32); hqmc_rng_gauss: the
+ * Gaussian pairs (d_out[2 n], fp64); hqmc_rng_uniform: the Metropolis uniform of update k (first uniform of element 0 of
+ * stream 2), computed on the host. */
+int hqmc_rng_raw(hqmc_ctx *ctx, unsigned long long seed, unsigned update, unsigned stream, long long n, unsigned *d_out);
+int hqmc_rng_gauss(hqmc_ctx *ctx, unsigned long long seed, unsigned update, unsigned stream, long long n, double *d_out);
+double hqmc_rng_uniform(unsigned long long seed, unsigned update);
+
+/* n_updates HQMC updates (the sweep loop of PAPER.md:183-201) on d_theta (in/out): update k = first_update + 0, 1, ...
+ * draws R (stream 0) and p (stream 1) on the device and u (stream 2), then runs steps (i)-(iv) as hqmc_hqmc_step does.
+ * H0_out, H1_out, accepted_out, cg_iters_out: HOST arrays of n_updates entries (may be NULL).  HQMC_ENOCONV if any solve
+ * missed cg_tol (the sweep still completes). */
+int hqmc_sweep(hqmc_ctx *ctx, double *d_theta, unsigned long long seed, unsigned first_update, int n_updates, int nsteps,
+               double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out, int *accepted_out,
+               long long *cg_iters_out);
+
 /* ---- Stochastic estimation of fermionic observables ----
  * All pointers are DEVICE pointers to lattice vectors [Ntau][L][L] of the context's complex type (n_rv of them back to
  * back where a count is given), 16-byte aligned, caller-owned.  The calls enqueue on the context's stream; cuFFT provides

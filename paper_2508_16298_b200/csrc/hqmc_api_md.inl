@@ -156,6 +156,49 @@ extern "C" int hqmc_hqmc_step(hqmc_ctx *c, double *d_theta, double *d_p, const v
 }
 
 // ---------------------------------------------------------------------------------------------------
+// on-device random numbers and the sweep loop
+// ---------------------------------------------------------------------------------------------------
+static int rng_grid(const hqmc_ctx *c, size_t n) { return (int)std::max<size_t>(1, std::min<size_t>((n + 255) / 256, (size_t)c->n_sm * 8)); }
+
+extern "C" int hqmc_rng_raw(hqmc_ctx *c, unsigned long long seed, unsigned update, unsigned stream, long long n, unsigned *d_out) {
+    if (!c || n < 0 || !aligned16(d_out)) return HQMC_EINVAL;
+    if (n == 0) return HQMC_OK;
+    return launch(c, HQMC_K_MISC, k_rng<double, 0>, dim3(rng_grid(c, (size_t)n)), dim3(256), 0, seed, (uint32_t)update, (uint32_t)stream, (size_t)n, (void *)d_out);
+}
+extern "C" int hqmc_rng_gauss(hqmc_ctx *c, unsigned long long seed, unsigned update, unsigned stream, long long n, double *d_out) {
+    if (!c || n < 0 || !aligned16(d_out)) return HQMC_EINVAL;
+    if (n == 0) return HQMC_OK;
+    return launch(c, HQMC_K_MISC, k_rng<double, 1>, dim3(rng_grid(c, (size_t)n)), dim3(256), 0, seed, (uint32_t)update, (uint32_t)stream, (size_t)n, (void *)d_out);
+}
+extern "C" double hqmc_rng_uniform(unsigned long long seed, unsigned update) {
+    const Philox4 b = rng_block(seed, (uint32_t)update, 2u, 0ull);
+    return rng_u53(b.x[0], b.x[1]);
+}
+
+extern "C" int hqmc_sweep(hqmc_ctx *c, double *d_theta, unsigned long long seed, unsigned first_update, int n_updates, int nsteps, double eps,
+                          double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out, int *accepted_out, long long *cg_iters_out) {
+    if (!c || !aligned16(d_theta) || n_updates < 0 || nsteps < 0 || cg_max_iter < 0) return HQMC_EINVAL;
+    int worst = HQMC_OK;
+    for (int k = 0; k < n_updates; ++k) {
+        const uint32_t upd = (uint32_t)first_update + (uint32_t)k;
+        // (i) R and p drawn on the device: R into the CG's z buffer (consumed by phi = M^+ R before the solver touches it),
+        //     p into the context's momentum buffer
+        if (c->prm.prec == HQMC_C128)
+            HQ_TRY(launch(c, HQMC_K_MISC, k_rng<double, 2>, dim3(rng_grid(c, c->N)), dim3(256), 0, seed, upd, 0u, c->N, c->d_z));
+        else
+            HQ_TRY(launch(c, HQMC_K_MISC, k_rng<float, 2>, dim3(rng_grid(c, c->N)), dim3(256), 0, seed, upd, 0u, c->N, c->d_z));
+        HQ_TRY(launch(c, HQMC_K_MISC, k_rng<double, 1>, dim3(rng_grid(c, c->N)), dim3(256), 0, seed, upd, 1u, c->N, (void *)c->d_p));
+        const double u = hqmc_rng_uniform(seed, upd);
+        // (ii)-(iv)
+        const int st = hqmc_hqmc_step(c, d_theta, c->d_p, c->d_z, u, nsteps, eps, cg_tol, cg_max_iter, H0_out ? H0_out + k : nullptr,
+                                      H1_out ? H1_out + k : nullptr, accepted_out ? accepted_out + k : nullptr,
+                                      cg_iters_out ? cg_iters_out + k : nullptr);
+        if (st == HQMC_ENOCONV) worst = st; else if (st != HQMC_OK) return st;
+    }
+    return worst;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // host-buffer variants: H2D copies, compute, D2H copies, all on the context's stream
 // ---------------------------------------------------------------------------------------------------
 extern "C" int hqmc_apply_MdagM_host(hqmc_ctx *c, const void *h_in, void *h_out) {

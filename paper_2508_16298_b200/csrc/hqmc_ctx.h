@@ -21,6 +21,7 @@
 #include "precond_tma.cuh"
 #include "measure_kernels.cuh"
 #include "cg_batched.cuh"
+#include "rng_kernels.cuh"
 
 namespace hqmc {
 

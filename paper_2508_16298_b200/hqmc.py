@@ -25,7 +25,7 @@ KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
-    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_rng_raw", "hqmc_rng_gauss", "hqmc_rng_uniform", "hqmc_sweep", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_variant", "hqmc_set_md_graph", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
@@ -47,6 +47,7 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 _lib.hqmc_strerror.restype = C.c_char_p
 _lib.hqmc_last_error.restype = C.c_char_p
+_lib.hqmc_rng_uniform.restype = C.c_double
 for _s in SYMBOLS:
     getattr(_lib, _s)  # raises AttributeError if a declared symbol is not exported
 
@@ -204,6 +205,33 @@ class HQMC:
                                        C.c_double(u), C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter),
                                        C.byref(H0), C.byref(H1), C.byref(acc), C.byref(it)), allow_noconv=True)
         return dict(H0=H0.value, H1=H1.value, accepted=bool(acc.value), cg_iters=it.value, converged=(s == HQMC_OK))
+
+    # ---- on-device random numbers and the sweep loop --------------------------
+    def rng_raw(self, seed, update, stream, n):
+        """The four Philox4x32-10 words of elements 0..n-1 -> uint32 tensor [n, 4] (bit-identical to the CPU twin)."""
+        out = torch.empty((n, 4), dtype=torch.int32, device=self.device)
+        _check(_lib.hqmc_rng_raw(self._ctx, C.c_ulonglong(seed), C.c_uint(update), C.c_uint(stream), C.c_longlong(n), _ptr(out)))
+        return out
+
+    def rng_gauss(self, seed, update, stream, n):
+        """n pairs of independent N(0, 1/2) -> float64 tensor [n, 2]."""
+        out = torch.empty((n, 2), dtype=torch.float64, device=self.device)
+        _check(_lib.hqmc_rng_gauss(self._ctx, C.c_ulonglong(seed), C.c_uint(update), C.c_uint(stream), C.c_longlong(n), _ptr(out)))
+        return out
+
+    @staticmethod
+    def rng_uniform(seed, update):
+        return float(_lib.hqmc_rng_uniform(C.c_ulonglong(seed), C.c_uint(update)))
+
+    def sweep(self, theta, seed, first_update, n_updates, nsteps, eps, cg_tol=1e-10, cg_max_iter=1000000):
+        """n_updates HQMC updates in place on theta, every random number drawn by the library
+        -> dict(H0[], H1[], accepted[], cg_iters[], converged)."""
+        n = n_updates
+        H0, H1, it, acc = (C.c_double * n)(), (C.c_double * n)(), (C.c_longlong * n)(), (C.c_int * n)()
+        s = _check(_lib.hqmc_sweep(self._ctx, _ptr(self._field(theta)), C.c_ulonglong(seed), C.c_uint(first_update), C.c_int(n),
+                                   C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter), H0, H1, acc, it),
+                   allow_noconv=True)
+        return dict(H0=list(H0), H1=list(H1), accepted=[bool(a) for a in acc], cg_iters=list(it), converged=(s == HQMC_OK))
 
     # ---- stochastic estimator (PAPER.md:220-244) -------------------------------------------------
     def _vecs(self, v):

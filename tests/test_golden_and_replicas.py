@@ -106,4 +106,5 @@ def test_bench_reference_arm_json_contract():
         assert k in line, k
     assert line["impl"] == "reference" and line["value"] > 0 and line["unit"] == "Gsite/s"
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
-    assert line["config"]["cg_iters_per_solve"] == 3
+    # `config` names the WORKLOAD (the GPU arm's: 500 fixed iterations per solve), `sample` what was run of it
+    assert line["config"]["cg_iters_per_solve"] == 500 and " 3 of its 500 " in line["cpu_baseline"]["sample"]

@@ -203,3 +203,37 @@ def test_leapfrog_step_graph_is_bitwise_identical_to_plain_launches(hq, L, Nt):
         g.close()
     assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
     assert out[0][2:] == out[1][2:] and out[0][4] == 70 * 5
+
+
+def test_device_random_numbers_match_the_cpu_twin_bit_for_bit(hq):
+    """NEXT-1 (reading C25): same (seed, update, stream, element) -> the same Philox4x32-10 words bit
+    for bit, hence the same 53-bit uniforms; the Gaussians differ only by the last bits of log / sincos."""
+    g = hq.HQMC(4, 8)
+    seed, upd, n = 0xC0FFEE1234567, 41, 100003
+    for stream in (0, 1, 2):
+        raw = g.rng_raw(seed, upd, stream, n).cpu().numpy().view(np.uint32)
+        assert np.array_equal(raw, orc.rng_raw(seed, upd, stream, n))
+        gg = g.rng_gauss(seed, upd, stream, n).cpu().numpy()
+        assert np.abs(gg - orc.rng_gauss(seed, upd, stream, n)).max() <= 1e-14
+    assert hq.HQMC.rng_uniform(seed, upd) == orc.rng_uniform(seed, upd, 2, 1)[0, 0]
+    z = g.rng_gauss(7, 0, 0, 1 << 20)
+    assert abs(float((z ** 2).sum(dim=1).mean()) - 1.0) < 4e-3 and abs(float(z.var()) - 0.5) < 3e-3      # E|R|^2 = 1, Var = 1/2
+    g.close()
+
+
+def test_sweep_acceptance_sequence_equals_the_oracles(hq):
+    """hqmc_sweep (steps (i)-(iv) looped, every draw made on the device) against the oracle's sweep from the same seed on a
+    short chain: same acceptance sequence, H0 and dH to 1e-8, final theta to 1e-9."""
+    L, Nt, seed, n_upd = 6, 10, 99, 6
+    theta = inputs.theta_uniform(L, Nt, 1)
+    o = orc.Oracle(L, Nt, c_tau=0.0, K=0.0)
+    g = hq.HQMC(L, Nt, c_tau=0.0, K=0.0)
+    ref = o.hqmc_sweep(theta, seed, 3, n_upd, 5, 0.2, cg_tol=1e-13)       # eps = 0.2: a mix of accepted and rejected updates
+    dth = dev(theta)
+    r = g.sweep(dth, seed, 3, n_upd, 5, 0.2, cg_tol=1e-13)
+    assert r["converged"] and r["accepted"] == list(ref["accepted"])
+    assert 0 < sum(r["accepted"]) < n_upd or n_upd < 2, r["accepted"]
+    assert np.abs(np.array(r["H0"]) - ref["H0"]).max() <= 1e-8
+    assert np.abs((np.array(r["H1"]) - np.array(r["H0"])) - (ref["H1"] - ref["H0"])).max() <= 1e-8
+    assert np.abs(dth.cpu().numpy() - ref["theta"]).max() <= 1e-9
+    g.close()
