@@ -63,11 +63,11 @@ __global__ void k_action_boson(Geo g, const double *__restrict__ theta, double c
     if (threadIdx.x == 0) part[blockIdx.x] = s;
 }
 
-// inverse of one normalised factor: (1 + T(P))^{-1} = (1 - T(P)) / (1 - |P|^2)
-template <typename T2> __device__ __forceinline__ void unrot(T2 &vi, T2 &vj, const T2 P) {
+// inverse of one normalised factor: (1 + T(P))^{-1} = (1 - T(P)) / (1 - |P|^2); |P|^2 = tanh^2(a) is a constant of the
+// factor's family, so s = 1 / (1 - tanh^2 a) = cosh^2 a comes in as a number (no division per bond)
+template <typename T2, typename TS> __device__ __forceinline__ void unrot(T2 &vi, T2 &vj, const T2 P, const TS s) {
     T2 m; m.x = -P.x; m.y = -P.y;
     rot(vi, vj, m);
-    auto s = 1 / (1 - (P.x * P.x + P.y * P.y));
     vi.x *= s; vi.y *= s; vj.x *= s; vj.y *= s;
 }
 // Re[ conj(L_i) (i P) R_j + conj(L_j) (-i conj(P)) R_i ]
@@ -77,14 +77,14 @@ template <typename T2> __device__ __forceinline__ double bond_term(const T2 Li, 
     return -((double)Li.x * Ay - (double)Li.y * Ax) + ((double)Lj.x * By - (double)Lj.y * Bx);
 }
 // one reverse step for the y-pairs / x-pairs of a block: R <- E^{-1} R, accumulate, Lv <- E Lv
-template <typename T2> __device__ __forceinline__ void rev_y(T2 (&R)[4], T2 (&Lv)[4], const T2 (&P)[2], double (&acc)[2]) {
-    unrot(R[0], R[2], P[0]); unrot(R[1], R[3], P[1]);
+template <typename T2, typename TS> __device__ __forceinline__ void rev_y(T2 (&R)[4], T2 (&Lv)[4], const T2 (&P)[2], double (&acc)[2], const TS s) {
+    unrot(R[0], R[2], P[0], s); unrot(R[1], R[3], P[1], s);
     acc[0] += bond_term(Lv[0], Lv[2], R[0], R[2], P[0]);
     acc[1] += bond_term(Lv[1], Lv[3], R[1], R[3], P[1]);
     rot(Lv[0], Lv[2], P[0]); rot(Lv[1], Lv[3], P[1]);
 }
-template <typename T2> __device__ __forceinline__ void rev_x(T2 (&R)[4], T2 (&Lv)[4], const T2 (&P)[2], double (&acc)[2]) {
-    unrot(R[0], R[1], P[0]); unrot(R[2], R[3], P[1]);
+template <typename T2, typename TS> __device__ __forceinline__ void rev_x(T2 (&R)[4], T2 (&Lv)[4], const T2 (&P)[2], double (&acc)[2], const TS s) {
+    unrot(R[0], R[1], P[0], s); unrot(R[2], R[3], P[1], s);
     acc[0] += bond_term(Lv[0], Lv[1], R[0], R[1], P[0]);
     acc[1] += bond_term(Lv[2], Lv[3], R[2], R[3], P[1]);
     rot(Lv[0], Lv[1], P[0]); rot(Lv[2], Lv[3], P[1]);
@@ -96,11 +96,16 @@ template <typename T2> __device__ __forceinline__ void rev_x(T2 (&R)[4], T2 (&Lv
 // Forward: R = prod_k (1 + T_k) X_t.  Then the factors are walked in reverse: R is un-swept
 // (R_{k-1} = E_k^{-1} R_k), the bond terms of family k are accumulated from (L_k, R_{k-1}), and
 // L_{k-1} = E_k L_k.  FUSE_P: p += -(dS_B + dS_F) * half_eps instead of writing dS_F.
+// The bosonic force of the fused kick is built from the link-phase table the kernel reads anyway (complex128 only): with
+// U = e^{i theta}, sin(theta_a - theta_b) = Im(U_a conj U_b) and sin(curl theta) = Im(U_x(s) U_y(s+x) conj(U_x(s+y)) conj(U_y(s))),
+// so the four sines per bond of dS_B/dtheta cost a few multiplications instead of four fp64 sin() calls;
+// sin(curl) is formed once per site of the slice into shared memory (every plaquette serves four bonds).
+// Dynamic shared memory: exchange buffers (4 nb elements) + 32 doubles + Vs doubles.
 // ------------------------------------------------------------------------------------------------
 template <typename T, int BPT, int MAXT, bool FUSE_P>
 __global__ void __launch_bounds__(MAXT) k_force(Geo g, const typename Cx<T>::type *__restrict__ ph, const typename Cx<T>::type *__restrict__ X, T C,
                         double *__restrict__ out, const double *__restrict__ theta, double half_eps, double c_tau,
-                        double K, int compact, int nkick) {
+                        double K, int compact, int nkick, double th_full, double th_half) {
     typedef typename Cx<T>::type T2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Exch<T2> ex; ex.buf = reinterpret_cast<T2 *>(smem_raw); ex.nb = g.nb; ex.parity = 0;
@@ -111,8 +116,22 @@ __global__ void __launch_bounds__(MAXT) k_force(Geo g, const typename Cx<T>::typ
         const size_t nv = (size_t)blockIdx.y * g.Vs * g.Nt;
         ph += 2 * nv; X += nv; out += 2 * nv; theta += 2 * nv;
     }
-    const int t = blockIdx.x, tn = (t + 1 == g.Nt) ? 0 : t + 1;
+    const int t = blockIdx.x, tn = (t + 1 == g.Nt) ? 0 : t + 1, tp = (t == 0) ? g.Nt - 1 : t - 1;
     const double sigma = (t == g.Nt - 1) ? -1.0 : 1.0;
+    constexpr bool PHASE_BOSON = FUSE_P && sizeof(T) == 8;          // boson force from the phase table (fp64 phases only)
+    double *Splaq = reinterpret_cast<double *>(smem_raw + sizeof(T2) * 4 * g.nb + 32 * sizeof(double));
+    const double i_half = 1.0 / (th_half * th_half), i_full = 1.0 / (th_full * th_full);
+    if (PHASE_BOSON) {                                             // sin(curl theta_t) for every site of the slice
+        const T2 *pht = ph + (size_t)t * 2 * g.Vs;
+        for (int s = threadIdx.x; s < g.Vs; s += blockDim.x) {
+            const int y = s / g.L, x = s - y * g.L, xp = (x + 1 == g.L) ? 0 : x + 1, yp = (y + 1 == g.L) ? 0 : y + 1;
+            const T2 ux = pht[s], uy1 = pht[g.Vs + y * g.L + xp], ux1 = pht[yp * g.L + x], uy = pht[g.Vs + s];
+            const double ax = (double)ux.x * uy1.x - (double)ux.y * uy1.y, ay = (double)ux.x * uy1.y + (double)ux.y * uy1.x;     // U_x(s) U_y(s+x)
+            const double bx = (double)ux1.x * uy.x - (double)ux1.y * uy.y, by = (double)ux1.x * uy.y + (double)ux1.y * uy.x;     // U_x(s+y) U_y(s)
+            Splaq[s] = (ay * bx - ax * by) * ((x & 1) ? i_half : i_full) * i_half;      // Im(a conj b) / (|U_x|^2 |U_y|^2)
+        }
+    }
+    const T s_half = (T)(1.0 / (1.0 - th_half * th_half)), s_full = (T)(1.0 / (1.0 - th_full * th_full));
     const T sC = (T)(-sigma) * C;
     T2 R[BPT][4], Lv[BPT][4];
     Phases<T2> P[BPT];
@@ -132,19 +151,19 @@ __global__ void __launch_bounds__(MAXT) k_force(Geo g, const typename Cx<T>::typ
         }
     // reverse walk: E4 | E3 E2 | E1 | E2 E3 | E4  (layouts OO, OE, EE, OE, OO)
 #pragma unroll
-    for (int k = 0; k < BPT; ++k) if (b[k].act) rev_y(R[k], Lv[k], P[k].p4, a4[k]);
+    for (int k = 0; k < BPT; ++k) if (b[k].act) rev_y(R[k], Lv[k], P[k].p4, a4[k], s_half);
     realign<BPT>(0, ex, b, R); realign<BPT>(0, ex, b, Lv);
 #pragma unroll
-    for (int k = 0; k < BPT; ++k) if (b[k].act) { rev_y(R[k], Lv[k], P[k].p3, a3[k]); rev_x(R[k], Lv[k], P[k].p2, a2[k]); }
+    for (int k = 0; k < BPT; ++k) if (b[k].act) { rev_y(R[k], Lv[k], P[k].p3, a3[k], s_half); rev_x(R[k], Lv[k], P[k].p2, a2[k], s_half); }
     realign<BPT>(1, ex, b, R); realign<BPT>(1, ex, b, Lv);
 #pragma unroll
-    for (int k = 0; k < BPT; ++k) if (b[k].act) rev_x(R[k], Lv[k], P[k].p1, a1[k]);
+    for (int k = 0; k < BPT; ++k) if (b[k].act) rev_x(R[k], Lv[k], P[k].p1, a1[k], s_full);
     realign<BPT>(2, ex, b, R); realign<BPT>(2, ex, b, Lv);
 #pragma unroll
-    for (int k = 0; k < BPT; ++k) if (b[k].act) { rev_x(R[k], Lv[k], P[k].p2, a2[k]); rev_y(R[k], Lv[k], P[k].p3, a3[k]); }
-    realign<BPT>(3, ex, b, R); realign<BPT>(3, ex, b, Lv);
+    for (int k = 0; k < BPT; ++k) if (b[k].act) { rev_x(R[k], Lv[k], P[k].p2, a2[k], s_half); rev_y(R[k], Lv[k], P[k].p3, a3[k], s_half); }
+    realign<BPT>(3, ex, b, R); realign<BPT>(3, ex, b, Lv);                    // (their barriers also publish Splaq)
 #pragma unroll
-    for (int k = 0; k < BPT; ++k) if (b[k].act) rev_y(R[k], Lv[k], P[k].p4, a4[k]);
+    for (int k = 0; k < BPT; ++k) if (b[k].act) rev_y(R[k], Lv[k], P[k].p4, a4[k], s_half);
     // write: every bond of the slice is owned by exactly one (thread, family) pair
     const double f = 2.0 * sigma * (double)C;
     double *o = out + (size_t)t * 2 * g.Vs;
@@ -153,14 +172,44 @@ __global__ void __launch_bounds__(MAXT) k_force(Geo g, const typename Cx<T>::typ
         if (b[k].act) {
             const int off[8] = {b[k].p4[0], b[k].p4[1], b[k].p3[0], b[k].p3[1], b[k].p2[0], b[k].p2[1], b[k].p1[0], b[k].p1[1]};
             const double val[8] = {a4[k][0], a4[k][1], a3[k][0], a3[k][1], a2[k][0], a2[k][1], a1[k][0], a1[k][1]};
+            // every global read of the epilogue first (the stores to o[] below would otherwise fence the later loads of o[])
+            double pv[8]; T2 Pp[8], Pn[8]; double thm[8], th0[8], thq[8];
+            if (FUSE_P) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    pv[j] = o[off[j]];
+                    if (PHASE_BOSON) {
+                        if (compact) { Pp[j] = ph[(size_t)tp * 2 * g.Vs + off[j]]; Pn[j] = ph[(size_t)tn * 2 * g.Vs + off[j]]; }
+                        else { thm[j] = theta[(size_t)tp * 2 * g.Vs + off[j]]; th0[j] = theta[(size_t)t * 2 * g.Vs + off[j]]; thq[j] = theta[(size_t)tn * 2 * g.Vs + off[j]]; }
+                    }
+                }
+            }
+            const T2 Pt[8] = {P[k].p4[0], P[k].p4[1], P[k].p3[0], P[k].p3[1], P[k].p2[0], P[k].p2[1], P[k].p1[0], P[k].p1[1]};
+            // site of each bond: the block's sites in the OO layout give (x, y) without a division
+            const int L = g.L, bq = b[k].q, by = bq / g.h, bx = bq - by * g.h, xa = 2 * bx + 1, xb = (xa + 1 == L) ? 0 : xa + 1, ya = 2 * by + 1;
+            const int bxs[8] = {xa, xb, xa, xb, xa, xa, 2 * bx, 2 * bx}, bys[8] = {ya, ya, 2 * by, 2 * by, 2 * by, 2 * by + 1, 2 * by, 2 * by + 1};
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 double gF = f * val[j];
                 if (FUSE_P) {
-                    double gB = dSB_bond(theta, g, t, off[j], c_tau, K, compact);
-                    double pv = o[off[j]];
-                    for (int n = 0; n < nkick; ++n) pv = fma(-(gB + gF), half_eps, pv);   // nkick half kicks with the same F (Eq.16)
-                    o[off[j]] = pv;
+                    double gB;
+                    if (PHASE_BOSON) {
+                        const int x = bxs[j], y = bys[j], sN = y * L + x;
+                        if (compact) {                    // c_tau [sin(theta_t - theta_{t-1}) - sin(theta_{t+1} - theta_t)]
+                            const double i2 = (j >= 6) ? i_full : i_half;              // family 1 (p1) carries tanh(a), the others tanh(a/2)
+                            const double sm = ((double)Pt[j].y * Pp[j].x - (double)Pt[j].x * Pp[j].y) * i2, sp = ((double)Pn[j].y * Pt[j].x - (double)Pn[j].x * Pt[j].y) * i2;
+                            gB = c_tau * (sm - sp);
+                        } else {
+                            gB = 2.0 * c_tau * ((th0[j] - thm[j]) - (thq[j] - th0[j]));
+                        }
+                        if (j >= 4) gB += -K * Splaq[sN] + K * Splaq[((y == 0) ? L - 1 : y - 1) * L + x];       // x-bonds (p2, p1)
+                        else        gB += K * Splaq[sN] - K * Splaq[y * L + ((x == 0) ? L - 1 : x - 1)];       // y-bonds (p4, p3)
+                    } else {
+                        gB = dSB_bond(theta, g, t, off[j], c_tau, K, compact);
+                    }
+                    double pvj = pv[j];
+                    for (int n = 0; n < nkick; ++n) pvj = fma(-(gB + gF), half_eps, pvj);   // nkick half kicks with the same F (Eq.16)
+                    o[off[j]] = pvj;
                 } else {
                     o[off[j]] = gF;
                 }

@@ -68,6 +68,7 @@ template <typename F> static int with_cfg(const hqmc_ctx *c, F &&f) {
 }
 
 static size_t block_smem(const hqmc_ctx *c) { return (size_t)4 * c->g.nb * c->esz + 32 * sizeof(double); }
+static size_t force_smem(const hqmc_ctx *c) { return block_smem(c) + (size_t)c->g.Vs * sizeof(double); }     // + sin(curl) per site
 
 template <typename T> static int set_attrs(hqmc_ctx *c) {
     const int smem = (int)block_smem(c);
@@ -78,8 +79,8 @@ template <typename T> static int set_attrs(hqmc_ctx *c) {
         CUDA_TRY(cudaFuncSetAttribute(k_apply_B<T, B, M>, attr, smem));
         CUDA_TRY(cudaFuncSetAttribute(k_mdagm<T, B, M, false>, attr, smem));
         CUDA_TRY(cudaFuncSetAttribute(k_mdagm<T, B, M, true>, attr, smem));
-        CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, false>, attr, smem));
-        CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, true>, attr, smem));
+        CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, false>, attr, (int)force_smem(c)));
+        CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, true>, attr, (int)force_smem(c)));
         if (c->use_stream) {
             CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, false>, attr, (int)c->stream_smem));
             CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, true>, attr, (int)c->stream_smem));
@@ -290,12 +291,12 @@ template <typename T> static int do_force(hqmc_ctx *c, const void *X, double *ou
     return with_cfg(c, [&](auto bpt, auto maxt) -> int {
         constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
         if (fuse_p)
-            return launch(c, HQMC_K_FORCE, k_force<T, B, M, true>, dim3(c->g.Nt), dim3(c->cfg.threads), block_smem(c), c->g,
+            return launch(c, HQMC_K_FORCE, k_force<T, B, M, true>, dim3(c->g.Nt), dim3(c->cfg.threads), force_smem(c), c->g,
                           (const T2 *)c->d_ph, (const T2 *)X, (T)c->C, out, (const double *)c->d_theta, half_eps,
-                          c->prm.c_tau, c->prm.K, c->prm.compact, nkick);
-        return launch(c, HQMC_K_FORCE, k_force<T, B, M, false>, dim3(c->g.Nt), dim3(c->cfg.threads), block_smem(c), c->g,
+                          c->prm.c_tau, c->prm.K, c->prm.compact, nkick, c->th_full, c->th_half);
+        return launch(c, HQMC_K_FORCE, k_force<T, B, M, false>, dim3(c->g.Nt), dim3(c->cfg.threads), force_smem(c), c->g,
                       (const T2 *)c->d_ph, (const T2 *)X, (T)c->C, out, (const double *)c->d_theta, 0.0, c->prm.c_tau,
-                      c->prm.K, c->prm.compact, 0);
+                      c->prm.K, c->prm.compact, 0, c->th_full, c->th_half);
     });
 }
 

@@ -35,9 +35,9 @@ template <typename T> static int traj_batched_t(hqmc_ctx *c, double *d_theta, do
     auto kick = [&](double half_eps, int nkick) -> int {
         return with_cfg(c, [&](auto bpt, auto maxt) -> int {
             constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
-            return launch(c, HQMC_K_FORCE, k_force<T, B, M, true>, dim3(c->g.Nt, n), dim3(c->cfg.threads), block_smem(c), c->g,
+            return launch(c, HQMC_K_FORCE, k_force<T, B, M, true>, dim3(c->g.Nt, n), dim3(c->cfg.threads), force_smem(c), c->g,
                           (const T2 *)c->d_cgb_ph, (const T2 *)X, (T)c->C, d_p, (const double *)d_theta, half_eps, c->prm.c_tau,
-                          c->prm.K, c->prm.compact, nkick);
+                          c->prm.K, c->prm.compact, nkick, c->th_full, c->th_half);
         });
     };
     auto energies = [&](int slot0) -> int {
