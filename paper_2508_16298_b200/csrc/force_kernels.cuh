@@ -90,6 +90,83 @@ template <typename T2, typename TS> __device__ __forceinline__ void rev_x(T2 (&R
     rot(Lv[0], Lv[1], P[0]); rot(Lv[2], Lv[3], P[1]);
 }
 
+// sin(curl theta_t) for every site of slice t from the link-phase table (all threads of the CTA; publish with a barrier):
+// Im(U_x(s) U_y(s+x) conj(U_x(s+y)) conj(U_y(s))) / (|U_x|^2 |U_y|^2), |U| = tanh(a) of the bond's family.
+template <typename T2>
+__device__ __forceinline__ void force_splaq(const Geo &g, const T2 *__restrict__ pht, double *__restrict__ Splaq, double i_half, double i_full) {
+    for (int s = threadIdx.x; s < g.Vs; s += blockDim.x) {
+        const int y = s / g.L, x = s - y * g.L, xp = (x + 1 == g.L) ? 0 : x + 1, yp = (y + 1 == g.L) ? 0 : y + 1;
+        const T2 ux = pht[s], uy1 = pht[g.Vs + y * g.L + xp], ux1 = pht[yp * g.L + x], uy = pht[g.Vs + s];
+        const double ax = (double)ux.x * uy1.x - (double)ux.y * uy1.y, ay = (double)ux.x * uy1.y + (double)ux.y * uy1.x;     // U_x(s) U_y(s+x)
+        const double bx = (double)ux1.x * uy.x - (double)ux1.y * uy.y, by = (double)ux1.x * uy.y + (double)ux1.y * uy.x;     // U_x(s+y) U_y(s)
+        Splaq[s] = (ay * bx - ax * by) * ((x & 1) ? i_half : i_full) * i_half;
+    }
+}
+
+// The write of one block's eight bonds (two per family: 4, 3, 2, 1): dS_F/dtheta = f val, or with FUSE_P the kick
+// p += -(dS_B + dS_F) half_eps (nkick times).  Pt: the block's link phases in the same order; (bx, by): the block.
+template <typename T, bool FUSE_P>
+__device__ __forceinline__ void force_write(const Geo &g, int t, int bx, int by, const typename Cx<T>::type (&Pt)[8], const double (&val)[8],
+                                            double f, const typename Cx<T>::type *__restrict__ ph, double *__restrict__ out,
+                                            const double *__restrict__ theta, const double *__restrict__ Splaq, double half_eps, double c_tau,
+                                            double K, int compact, int nkick, double i_half, double i_full) {
+    typedef typename Cx<T>::type T2;
+    constexpr bool PHASE_BOSON = FUSE_P && sizeof(T) == 8;
+    const int L = g.L, Vs = g.Vs;
+    const int tn = (t + 1 == g.Nt) ? 0 : t + 1, tp = (t == 0) ? g.Nt - 1 : t - 1;
+    const int xa = 2 * bx + 1, xb = (xa + 1 == L) ? 0 : xa + 1, ya = 2 * by + 1;
+    // site of each bond (block_engine.cuh make_block): y-bonds (xa,ya) (xb,ya) (xa,2by) (xb,2by), x-bonds (xa,2by) (xa,2by+1) (2bx,2by) (2bx,2by+1)
+    const int bxs[8] = {xa, xb, xa, xb, xa, xa, 2 * bx, 2 * bx}, bys[8] = {ya, ya, 2 * by, 2 * by, 2 * by, 2 * by + 1, 2 * by, 2 * by + 1};
+    int off[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) off[j] = (j < 4 ? Vs : 0) + bys[j] * L + bxs[j];
+    double *o = out + (size_t)t * 2 * Vs;
+    // two groups of four bonds (y-bonds, then x-bonds): the group's global reads first, in one batch (the stores to o[] would
+    // otherwise fence the later loads of o[]); four at a time keeps the batch within the register budget
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        double pv[4]; T2 Pp[4], Pn[4]; double thm[4], th0[4], thq[4];
+        if (FUSE_P) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int j = 4 * h + i;
+                pv[i] = o[off[j]];
+                if (PHASE_BOSON) {
+                    if (compact) { Pp[i] = ph[(size_t)tp * 2 * Vs + off[j]]; Pn[i] = ph[(size_t)tn * 2 * Vs + off[j]]; }
+                    else { thm[i] = theta[(size_t)tp * 2 * Vs + off[j]]; th0[i] = theta[(size_t)t * 2 * Vs + off[j]]; thq[i] = theta[(size_t)tn * 2 * Vs + off[j]]; }
+                }
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int j = 4 * h + i;
+            const double gF = f * val[j];
+            if (FUSE_P) {
+                double gB;
+                if (PHASE_BOSON) {
+                    const int x = bxs[j], y = bys[j], sN = y * L + x;
+                    if (compact) {                    // c_tau [sin(theta_t - theta_{t-1}) - sin(theta_{t+1} - theta_t)]
+                        const double i2 = (j >= 6) ? i_full : i_half;              // family 1 carries tanh(a), the others tanh(a/2)
+                        const double sm = ((double)Pt[j].y * Pp[i].x - (double)Pt[j].x * Pp[i].y) * i2, sp = ((double)Pn[i].y * Pt[j].x - (double)Pn[i].x * Pt[j].y) * i2;
+                        gB = c_tau * (sm - sp);
+                    } else {
+                        gB = 2.0 * c_tau * ((th0[i] - thm[i]) - (thq[i] - th0[i]));
+                    }
+                    if (h == 1) gB += -K * Splaq[sN] + K * Splaq[((y == 0) ? L - 1 : y - 1) * L + x];       // x-bonds
+                    else        gB += K * Splaq[sN] - K * Splaq[y * L + ((x == 0) ? L - 1 : x - 1)];       // y-bonds
+                } else {
+                    gB = dSB_bond(theta, g, t, off[j], c_tau, K, compact);
+                }
+                double pvj = pv[i];
+                for (int n = 0; n < nkick; ++n) pvj = fma(-(gB + gF), half_eps, pvj);   // nkick half kicks with the same F (Eq.16)
+                o[off[j]] = pvj;
+            } else {
+                o[off[j]] = gF;
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // S9 (+S10): one CTA per slice t.
 //   dS_F/dtheta_{b,t} = 2 sigma_t Re[ Y_{t+1}^+ (dB_t/dtheta_b) X_t ],  Y_{t+1} = X_{t+1} - sigma_t B_t X_t.
@@ -116,21 +193,12 @@ __global__ void __launch_bounds__(MAXT) k_force(Geo g, const typename Cx<T>::typ
         const size_t nv = (size_t)blockIdx.y * g.Vs * g.Nt;
         ph += 2 * nv; X += nv; out += 2 * nv; theta += 2 * nv;
     }
-    const int t = blockIdx.x, tn = (t + 1 == g.Nt) ? 0 : t + 1, tp = (t == 0) ? g.Nt - 1 : t - 1;
+    const int t = blockIdx.x, tn = (t + 1 == g.Nt) ? 0 : t + 1;
     const double sigma = (t == g.Nt - 1) ? -1.0 : 1.0;
     constexpr bool PHASE_BOSON = FUSE_P && sizeof(T) == 8;          // boson force from the phase table (fp64 phases only)
     double *Splaq = reinterpret_cast<double *>(smem_raw + sizeof(T2) * 4 * g.nb + 32 * sizeof(double));
     const double i_half = 1.0 / (th_half * th_half), i_full = 1.0 / (th_full * th_full);
-    if (PHASE_BOSON) {                                             // sin(curl theta_t) for every site of the slice
-        const T2 *pht = ph + (size_t)t * 2 * g.Vs;
-        for (int s = threadIdx.x; s < g.Vs; s += blockDim.x) {
-            const int y = s / g.L, x = s - y * g.L, xp = (x + 1 == g.L) ? 0 : x + 1, yp = (y + 1 == g.L) ? 0 : y + 1;
-            const T2 ux = pht[s], uy1 = pht[g.Vs + y * g.L + xp], ux1 = pht[yp * g.L + x], uy = pht[g.Vs + s];
-            const double ax = (double)ux.x * uy1.x - (double)ux.y * uy1.y, ay = (double)ux.x * uy1.y + (double)ux.y * uy1.x;     // U_x(s) U_y(s+x)
-            const double bx = (double)ux1.x * uy.x - (double)ux1.y * uy.y, by = (double)ux1.x * uy.y + (double)ux1.y * uy.x;     // U_x(s+y) U_y(s)
-            Splaq[s] = (ay * bx - ax * by) * ((x & 1) ? i_half : i_full) * i_half;      // Im(a conj b) / (|U_x|^2 |U_y|^2)
-        }
-    }
+    if (PHASE_BOSON) force_splaq(g, ph + (size_t)t * 2 * g.Vs, Splaq, i_half, i_full);
     const T s_half = (T)(1.0 / (1.0 - th_half * th_half)), s_full = (T)(1.0 / (1.0 - th_full * th_full));
     const T sC = (T)(-sigma) * C;
     T2 R[BPT][4], Lv[BPT][4];
@@ -166,54 +234,13 @@ __global__ void __launch_bounds__(MAXT) k_force(Geo g, const typename Cx<T>::typ
     for (int k = 0; k < BPT; ++k) if (b[k].act) rev_y(R[k], Lv[k], P[k].p4, a4[k], s_half);
     // write: every bond of the slice is owned by exactly one (thread, family) pair
     const double f = 2.0 * sigma * (double)C;
-    double *o = out + (size_t)t * 2 * g.Vs;
 #pragma unroll
     for (int k = 0; k < BPT; ++k)
         if (b[k].act) {
-            const int off[8] = {b[k].p4[0], b[k].p4[1], b[k].p3[0], b[k].p3[1], b[k].p2[0], b[k].p2[1], b[k].p1[0], b[k].p1[1]};
-            const double val[8] = {a4[k][0], a4[k][1], a3[k][0], a3[k][1], a2[k][0], a2[k][1], a1[k][0], a1[k][1]};
-            // every global read of the epilogue first (the stores to o[] below would otherwise fence the later loads of o[])
-            double pv[8]; T2 Pp[8], Pn[8]; double thm[8], th0[8], thq[8];
-            if (FUSE_P) {
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    pv[j] = o[off[j]];
-                    if (PHASE_BOSON) {
-                        if (compact) { Pp[j] = ph[(size_t)tp * 2 * g.Vs + off[j]]; Pn[j] = ph[(size_t)tn * 2 * g.Vs + off[j]]; }
-                        else { thm[j] = theta[(size_t)tp * 2 * g.Vs + off[j]]; th0[j] = theta[(size_t)t * 2 * g.Vs + off[j]]; thq[j] = theta[(size_t)tn * 2 * g.Vs + off[j]]; }
-                    }
-                }
-            }
             const T2 Pt[8] = {P[k].p4[0], P[k].p4[1], P[k].p3[0], P[k].p3[1], P[k].p2[0], P[k].p2[1], P[k].p1[0], P[k].p1[1]};
-            // site of each bond: the block's sites in the OO layout give (x, y) without a division
-            const int L = g.L, bq = b[k].q, by = bq / g.h, bx = bq - by * g.h, xa = 2 * bx + 1, xb = (xa + 1 == L) ? 0 : xa + 1, ya = 2 * by + 1;
-            const int bxs[8] = {xa, xb, xa, xb, xa, xa, 2 * bx, 2 * bx}, bys[8] = {ya, ya, 2 * by, 2 * by, 2 * by, 2 * by + 1, 2 * by, 2 * by + 1};
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                double gF = f * val[j];
-                if (FUSE_P) {
-                    double gB;
-                    if (PHASE_BOSON) {
-                        const int x = bxs[j], y = bys[j], sN = y * L + x;
-                        if (compact) {                    // c_tau [sin(theta_t - theta_{t-1}) - sin(theta_{t+1} - theta_t)]
-                            const double i2 = (j >= 6) ? i_full : i_half;              // family 1 (p1) carries tanh(a), the others tanh(a/2)
-                            const double sm = ((double)Pt[j].y * Pp[j].x - (double)Pt[j].x * Pp[j].y) * i2, sp = ((double)Pn[j].y * Pt[j].x - (double)Pn[j].x * Pt[j].y) * i2;
-                            gB = c_tau * (sm - sp);
-                        } else {
-                            gB = 2.0 * c_tau * ((th0[j] - thm[j]) - (thq[j] - th0[j]));
-                        }
-                        if (j >= 4) gB += -K * Splaq[sN] + K * Splaq[((y == 0) ? L - 1 : y - 1) * L + x];       // x-bonds (p2, p1)
-                        else        gB += K * Splaq[sN] - K * Splaq[y * L + ((x == 0) ? L - 1 : x - 1)];       // y-bonds (p4, p3)
-                    } else {
-                        gB = dSB_bond(theta, g, t, off[j], c_tau, K, compact);
-                    }
-                    double pvj = pv[j];
-                    for (int n = 0; n < nkick; ++n) pvj = fma(-(gB + gF), half_eps, pvj);   // nkick half kicks with the same F (Eq.16)
-                    o[off[j]] = pvj;
-                } else {
-                    o[off[j]] = gF;
-                }
-            }
+            const double val[8] = {a4[k][0], a4[k][1], a3[k][0], a3[k][1], a2[k][0], a2[k][1], a1[k][0], a1[k][1]};
+            const int by = b[k].q / g.h, bx = b[k].q - by * g.h;
+            force_write<T, FUSE_P>(g, t, bx, by, Pt, val, f, ph, out, theta, Splaq, half_eps, c_tau, K, compact, nkick, i_half, i_full);
         }
 }
 

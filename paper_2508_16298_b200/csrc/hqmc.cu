@@ -82,6 +82,8 @@ template <typename T> static int set_attrs(hqmc_ctx *c) {
         CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, false>, attr, (int)force_smem(c)));
         CUDA_TRY(cudaFuncSetAttribute(k_force<T, B, M, true>, attr, (int)force_smem(c)));
         if (c->use_stream) {
+            CUDA_TRY(cudaFuncSetAttribute(k_force_stream<T, false>, attr, (int)c->force_stream_smem));
+            CUDA_TRY(cudaFuncSetAttribute(k_force_stream<T, true>, attr, (int)c->force_stream_smem));
             CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, false>, attr, (int)c->stream_smem));
             CUDA_TRY(cudaFuncSetAttribute(k_mdagm_back<T, true>, attr, (int)c->stream_smem));
         }
@@ -288,6 +290,17 @@ template <typename T> static int do_precond(hqmc_ctx *c, const void *in, void *o
 
 template <typename T> static int do_force(hqmc_ctx *c, const void *X, double *out, bool fuse_p, double half_eps, int nkick) {
     typedef typename Cx<T>::type T2;
+    typedef typename PhasePack<T>::word W;
+    if (c->use_stream && c->stream_on) {             // streaming form: one CTA per SM over a run of slices (force_stream.cuh)
+        const int G = c->g.Nt < c->n_sm ? c->g.Nt : c->n_sm;
+        if (fuse_p)
+            return launch(c, HQMC_K_FORCE, k_force_stream<T, true>, dim3(G), dim3(c->cfg.threads), c->force_stream_smem, c->g,
+                          (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)c->d_ph, (const T2 *)X, (T)c->C, out,
+                          (const double *)c->d_theta, half_eps, c->prm.c_tau, c->prm.K, c->prm.compact, nkick, c->th_full, c->th_half);
+        return launch(c, HQMC_K_FORCE, k_force_stream<T, false>, dim3(G), dim3(c->cfg.threads), c->force_stream_smem, c->g,
+                      (const W *)c->d_packed, (const double2 *)c->d_tab, (const T2 *)c->d_ph, (const T2 *)X, (T)c->C, out,
+                      (const double *)c->d_theta, 0.0, c->prm.c_tau, c->prm.K, c->prm.compact, 0, c->th_full, c->th_half);
+    }
     return with_cfg(c, [&](auto bpt, auto maxt) -> int {
         constexpr int B = decltype(bpt)::value, M = decltype(maxt)::value;
         if (fuse_p)

@@ -100,6 +100,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     {   // streaming M^+M kernel (k_mdagm_back): one thread per 2x2 block and its staging buffers must fit one SM's shared memory
         const size_t need = (prm->prec == HQMC_C128) ? BackSmem<double>(c->g.Vs, c->cfg.threads).total : BackSmem<float>(c->g.Vs, c->cfg.threads).total;
         c->stream_smem = need;
+        c->force_stream_smem = (prm->prec == HQMC_C128) ? ForceSmem<double>(c->g.Vs, c->cfg.threads).total : ForceSmem<float>(c->g.Vs, c->cfg.threads).total;
         c->use_stream = (c->cfg.bpt == 1) && need <= (size_t)prop.sharedMemPerBlockOptin && (size_t)c->g.Vs * 16 < (1u << 20);
         c->stream_on = c->use_stream;
         // cluster kernel: the slice split over R SMs (smallest R whose strip fits one SM's threads and shared memory)

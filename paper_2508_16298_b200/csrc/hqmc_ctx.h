@@ -14,6 +14,7 @@
 #include "../../include/hqmc_tuning.h"
 #include "cg_kernels.cuh"
 #include "force_kernels.cuh"
+#include "force_stream.cuh"
 #include "kernels.cuh"
 #include "mdagm_stream.cuh"
 #include "mdagm_cluster.cuh"
@@ -76,6 +77,7 @@ struct hqmc_ctx {
     int cl_R, cl_threads; size_t cl_smem;
     bool use_stream;     // streaming kernel usable (one block per thread and its staging buffers fit one SM)
     size_t stream_smem;
+    size_t force_stream_smem = 0;   // k_force_stream (follows stream_on)
     void *d_r, *d_z, *d_d, *d_Od, *d_X, *d_phi;   // CG vectors, trajectory solution / pseudofermion
     double *d_p, *d_force;                        // host-variant staging
     double *d_part_dOd, *d_part_rr, *d_part_rz[2], *d_part_misc;
