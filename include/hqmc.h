@@ -208,6 +208,22 @@ int hqmc_leapfrog_trajectory_host(hqmc_ctx *ctx, double *h_theta, double *h_p, c
                                   double eps, double cg_tol, long long cg_max_iter, double *H0_out,
                                   double *H1_out, long long *cg_iters_out);
 
+/* ALLOCATION-FREE S_B (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it).  S_B(theta) of PAPER.md:52-54 (the same sum hqmc_energies returns as SB_out) written to the
+ * DEVICE double d_SB_out[0], with no context: the call allocates nothing -- no cudaMalloc, cudaFree or allocating library
+ * routine -- and enqueues two kernels on cuda_stream (a cudaStream_t of the CURRENT device; NULL = the default stream)
+ * without synchronising.  d_theta: device, fp64 [Ntau][2][L][L], read only; c_tau, K, compact as in hqmc_params; any
+ * L >= 2 (odd allowed), Ntau >= 1.  The per-CTA partial sums live in a static device array inside the library (64 KB, held
+ * by every GPU that loads the library until exit) with room for HQMC_NOALLOC_MAX_LINKS = 2^25 links: a lattice with
+ * 2 L^2 Ntau beyond that is rejected with HQMC_EINVAL and a message in hqmc_last_error (config 5, L = 64, Ntau = 640, has
+ * 5.2 M links).  Every call shares the array: calls whose kernels OVERLAP on the GPU (different streams without an event
+ * between them, or two host threads) race on it and may both return wrong sums; calls on one stream are safe.  Nothing in
+ * the array needs clearing between calls (each call writes every partial it reads).  The sum order differs from
+ * hqmc_energies (fixed 4096-link CTAs): results agree to rounding (~1e-14 relative), not bit for bit. */
+#define HQMC_NOALLOC_MAX_LINKS (1 << 25)
+int hqmc_action_boson_noalloc(const double *d_theta, int L, int Ntau, double c_tau, double K, int compact,
+                              double *d_SB_out, void *cuda_stream);
+
 /* Instrumentation and tuning knobs (launch statistics, kernel selection, timing experiments) are declared in
  * hqmc_tuning.h; nothing in this header depends on them. */
 

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhqmc.so")
-SOURCES = ["hqmc.cu"]
+SOURCES = ["hqmc.cu", "hqmc_noalloc.cu"]      # hqmc_noalloc.cu: self-contained (the allocation-free S_B entry point)
 HEADER = os.path.join("..", "..", "include", "hqmc.h")
 
 

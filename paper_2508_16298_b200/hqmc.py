@@ -27,7 +27,7 @@ SYMBOLS = [
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
     "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_rng_raw", "hqmc_rng_gauss", "hqmc_rng_uniform", "hqmc_sweep", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
-    "hqmc_leapfrog_trajectory_host", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
+    "hqmc_leapfrog_trajectory_host", "hqmc_action_boson_noalloc", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_variant", "hqmc_set_md_graph", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
 
@@ -361,3 +361,22 @@ class HQMC:
 
 def version() -> int:
     return int(_lib.hqmc_version())
+
+
+NOALLOC_MAX_LINKS = 1 << 25
+
+
+def action_boson_noalloc(theta: torch.Tensor, L: int, Nt: int, c_tau: float, K: float, compact: bool, out: torch.Tensor,
+                         stream=None) -> torch.Tensor:
+    """S_B(theta) into the caller's device double out[0] through hqmc_action_boson_noalloc (include/hqmc.h): no context and
+    no allocation anywhere -- the caller brings theta (fp64 [Nt][2][L][L], CUDA, contiguous) AND out (fp64, >= 1 element,
+    CUDA).  Enqueued on `stream` (default: torch's current stream), not synchronised.  Lattices beyond NOALLOC_MAX_LINKS
+    raise HqmcError; calls that overlap on the GPU race on the library's shared static scratch."""
+    if not (theta.is_cuda and out.is_cuda and theta.dtype == torch.float64 and out.dtype == torch.float64
+            and theta.is_contiguous() and out.numel() >= 1 and theta.numel() == 2 * L * L * Nt):
+        raise ValueError("theta: contiguous CUDA fp64 [Nt][2][L][L]; out: CUDA fp64 with at least one element")
+    st = torch.cuda.current_stream(theta.device).cuda_stream if stream is None else int(stream)
+    with torch.cuda.device(theta.device):
+        _check(_lib.hqmc_action_boson_noalloc(_ptr(theta), C.c_int(L), C.c_int(Nt), C.c_double(c_tau), C.c_double(K),
+                                              C.c_int(1 if compact else 0), _ptr(out), C.c_void_p(st)))
+    return out
