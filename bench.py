@@ -520,6 +520,82 @@ def run_solve(args):
     return 0
 
 
+def run_slab(args):
+    """--mode slab: the tau-slab path (paper_2508_16298_b200/slab.py) -- us per PCG iteration with
+    the lattice cut into S slabs, fixed iteration count.  One process: S = 1, 2, 4 slabs on the one GPU, slab after
+    slab (what sharding costs in halo slices, extra launches and host time, with no link in the way).  Under torchrun with N
+    ranks: one slab per rank, halos and sums over NCCL, time = max over ranks."""
+    import torch
+    from paper_2508_16298_b200 import hqmc, inputs
+    from paper_2508_16298_b200.slab import CudaSlabOps, SlabLayout, SlabSolver
+    rank, world, local = dist_env()
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    c = inputs.CONFIGS[args.config]
+    L, Ntau = (args.L, 10 * args.L) if args.L else (c["L"], c["Ntau"])
+    iters = args.cg_iters
+    theta = inputs.theta_uniform(L, Ntau, c["seed"])
+    eta = inputs.complex_gaussian((Ntau, L, L), c["seed"])
+    out = {"mode": "slab", "L": L, "Ntau": Ntau, "iters": iters, "n_gpus": world, "theta": "uniform", "slabs": {}}
+    dev = torch.device("cuda", local)
+    if rank == 0:
+        g = hqmc.HQMC(L, Ntau, device=dev)
+        g.set_theta(torch.from_numpy(theta).to(dev))
+        phi1 = g.apply_Mdag(torch.from_numpy(eta).to(dev))
+        g.cg_solve(phi1, 0.0, iters)
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        x1, _, rel1, _ = g.cg_solve(phi1, 0.0, iters)
+        torch.cuda.synchronize()
+        out["one_context"] = {"us_per_iter": 1e6 * (time.perf_counter() - t0) / iters, "relres": rel1}
+        phi_h = phi1.cpu().numpy()
+        x1_h = x1.cpu().numpy()
+        g.close()
+    else:
+        phi_h = None
+    if world > 1:
+        import torch.distributed as dist
+        box = [phi_h]
+        dist.broadcast_object_list(box, src=0)
+        phi_h = box[0]
+    for S in ([world] if world > 1 else [1, 2, 4]):
+        lay = SlabLayout(L, Ntau, S, W=6, world=world, rank=rank)
+        ops = CudaSlabOps(lay, device=dev)
+        sol = SlabSolver(lay, ops)
+        part = lambda a: [torch.from_numpy(np.ascontiguousarray(a[lay.bounds[gg]:lay.bounds[gg + 1]])).to(dev) for gg in lay.owned]
+        sol.set_theta(part(theta))
+        rhs = sol.extend(part(phi_h), ops.new_vec)
+        xs = [ops.new_vec(i) for i in range(len(lay.owned))]
+        res = {}
+        for graph in (False, True):
+            sol.solve(rhs, xs, 0.0, min(iters, 20), graph=graph)
+            torch.cuda.synchronize()
+            if world > 1:
+                torch.distributed.barrier()
+            t0 = time.perf_counter()
+            it, rel, _ = sol.solve(rhs, xs, 0.0, iters, graph=graph)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            if world > 1:
+                t = torch.tensor([dt], dtype=torch.float64, device=dev)
+                torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+                dt = float(t)
+            res["graph" if graph else "plain"] = {"us_per_iter": 1e6 * dt / it, "relres": rel}
+        if rank == 0 and world == 1:
+            x = np.concatenate([sol.own(v, i).cpu().numpy() for i, v in enumerate(xs)], axis=0)
+            res["max_rel_diff_vs_one_context"] = float(np.abs(x - x1_h).max() / np.abs(x1_h).max())
+        res["halo_slices_per_slab"] = 2 * lay.H
+        res["owned_slices"] = [lay.nt(gg) for gg in range(S)]
+        out["slabs"][str(S)] = res
+        ops.close()
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
 def run_trajectory(args):
     """--mode trajectory: BASELINE config 5's protocol ("5 HMC trajectories of 20 leapfrog steps each, reporting ms per
     trajectory and HBM fraction") on the chosen config.  The PCG runs the paper's fixed iteration count per solve
@@ -701,7 +777,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip cg_solve / c64 / config5 / md_graph keys (converged solves, second lattice)")
     ap.add_argument("--no-solve", action="store_true", help="skip the converged config-4 solves (about 20 s of GPU time)")
     ap.add_argument("--no-config5", action="store_true", help="skip the L=64 lattice (its heat-bath field costs 40 s of host time)")
-    ap.add_argument("--mode", default="step", choices=["step", "solve", "measure", "trajectory"],
+    ap.add_argument("--mode", default="step", choices=["step", "solve", "measure", "trajectory", "slab"],
                     help="solve: one full PCG solve to --tol; measure: the stochastic estimator on a paper-regime field (neither is the timed metric)")
     ap.add_argument("--n-traj", type=int, default=5, help="trajectory mode: timed trajectories (BASELINE config 5: 5)")
     ap.add_argument("--md-steps", type=int, default=20, help="trajectory mode: leapfrog steps per trajectory (BASELINE config 5: 20)")
@@ -723,6 +799,8 @@ def main():
         return run_measure(args)
     if args.mode == "trajectory":
         return run_trajectory(args)
+    if args.mode == "slab":
+        return run_slab(args)
     return run_reference(args) if args.impl == "reference" else run_gpu(args)
 
 

@@ -196,6 +196,31 @@ int hqmc_green_2pt(hqmc_ctx *ctx, const void *d_g, const void *d_xi, int n_rv, v
  * every unordered pair of the n_rv >= 2 vectors, mean over the binom(n_rv, 2) pairs. */
 int hqmc_pair_correlator(hqmc_ctx *ctx, const void *d_g, const void *d_xi, int n_rv, void *d_C);
 
+/* ---- tau-slab sharding (the paper is single-GPU) ----
+ * M and M^+ couple slice t only to t -+ 1 and the preconditioner to t +- W (PAPER.md:155 Eq.8, :316-326), so the lattice shards
+ * into contiguous runs of time slices.  A rank (or each of the slabs one process owns) creates an ordinary context for its
+ * EXTENDED lattice -- its nt_loc owned slices with H = max(1, W) halo slices on either side, Ntau = nt_loc + 2 H -- and sets the
+ * extended theta (the neighbours' slices in the halo).  With the halo slices of a vector filled from the neighbours, multiplied
+ * by -1 where they crossed the antiperiodic boundary (tau = Ntau_global - 1 -> 0), hqmc_apply_M / _Mdag / _MdagM, hqmc_precond
+ * and hqmc_force of that context return on the OWNED slices exactly what the global operators return (the extended lattice's
+ * own wrap only reaches its outermost halo slices, which are discarded).  What is left of a PCG iteration (Eq.20) are the
+ * vector updates and the inner products over the owned range, which is one contiguous run of n elements: the calls below,
+ * whose coefficients are quotients of DEVICE scalars (sums the ranks have all-reduced), so an iteration is enqueued without the
+ * host reading a number.  All pointers are device pointers, vectors 16-byte aligned; everything is enqueued on the context's
+ * stream, nothing synchronises.  The exchange itself (NCCL send/recv and all-reduce through torch.distributed) and the loop
+ * are paper_2508_16298_b200/slab.py. */
+/* d_out[0] = Re <a, b> over n elements (two-stage, fixed order). */
+int hqmc_slab_dot(hqmc_ctx *ctx, const void *d_a, const void *d_b, long long n, double *d_out);
+/* alpha = *d_num / *d_den;  x += alpha d;  r -= alpha Od;  d_rr_out[0] = ||r||^2 over the n elements. */
+int hqmc_slab_axpy(hqmc_ctx *ctx, void *d_x, void *d_r, const void *d_d, const void *d_Od, long long n,
+                   const double *d_num, const double *d_den, double *d_rr_out);
+/* beta = *d_num / *d_den;  d = z + beta d. */
+int hqmc_slab_dupdate(hqmc_ctx *ctx, void *d_d, const void *d_z, long long n, const double *d_num, const double *d_den);
+/* v *= s over n elements (s = -1: a halo that crossed the antiperiodic boundary; reading C1). */
+int hqmc_slab_scale(hqmc_ctx *ctx, void *d_v, long long n, double s);
+/* d_out[j] = sum_i d_in[i * stride + j], i < rows in order, j < cols: the partial sums of the slabs one process owns. */
+int hqmc_slab_sum_rows(hqmc_ctx *ctx, const double *d_in, int rows, int stride, int cols, double *d_out);
+
 /* HOST-buffer variants (pageable or pinned host memory; the copies run inside the call on the
  * context's stream and the call returns after the result has landed in h_out / h_x). */
 int hqmc_apply_MdagM_host(hqmc_ctx *ctx, const void *h_in, void *h_out);

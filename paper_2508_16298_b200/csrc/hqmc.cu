@@ -327,3 +327,4 @@ using namespace hqmc;
 #include "hqmc_api_md.inl"
 #include "hqmc_api_mdb.inl"
 #include "hqmc_api_measure.inl"
+#include "hqmc_api_slab.inl"

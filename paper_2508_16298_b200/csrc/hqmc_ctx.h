@@ -23,6 +23,7 @@
 #include "measure_kernels.cuh"
 #include "cg_batched.cuh"
 #include "rng_kernels.cuh"
+#include "slab_kernels.cuh"
 
 namespace hqmc {
 

@@ -27,7 +27,8 @@ SYMBOLS = [
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
     "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_rng_raw", "hqmc_rng_gauss", "hqmc_rng_uniform", "hqmc_sweep", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
-    "hqmc_leapfrog_trajectory_host", "hqmc_action_boson_noalloc", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
+    "hqmc_leapfrog_trajectory_host", "hqmc_action_boson_noalloc", "hqmc_slab_dot", "hqmc_slab_axpy", "hqmc_slab_dupdate",
+    "hqmc_slab_scale", "hqmc_slab_sum_rows", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_variant", "hqmc_set_md_graph", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
 
@@ -314,6 +315,32 @@ class HQMC:
         out = self.new_vec() if out is None else out
         _check(_lib.hqmc_pair_correlator(self._ctx, _ptr(g), _ptr(xi), C.c_int(n), _ptr(self._vec(out))))
         return out
+
+    # ---- vector steps of the tau-slab PCG (include/hqmc.h "tau-slab sharding"; the loop is slab.py) --------------
+    def slab_dot(self, a, b, out):
+        """out[0] = Re <a, b> over the (contiguous) views a, b; out: a device float64 view."""
+        assert a.is_contiguous() and b.is_contiguous() and a.numel() == b.numel() and a.dtype == b.dtype == self.cdtype
+        _check(_lib.hqmc_slab_dot(self._ctx, _ptr(a), _ptr(b), C.c_longlong(a.numel()), _ptr(out)))
+
+    def slab_axpy(self, x, r, d, Od, num, den, rr_out):
+        for v in (x, r, d, Od):
+            assert v.is_contiguous() and v.dtype == self.cdtype and v.numel() == x.numel()
+        _check(_lib.hqmc_slab_axpy(self._ctx, _ptr(x), _ptr(r), _ptr(d), _ptr(Od), C.c_longlong(x.numel()), _ptr(num), _ptr(den),
+                                   _ptr(rr_out)))
+
+    def slab_dupdate(self, d, z, num, den):
+        assert d.is_contiguous() and z.is_contiguous() and d.numel() == z.numel() and d.dtype == z.dtype == self.cdtype
+        _check(_lib.hqmc_slab_dupdate(self._ctx, _ptr(d), _ptr(z), C.c_longlong(d.numel()), _ptr(num), _ptr(den)))
+
+    def slab_scale(self, v, s):
+        assert v.is_contiguous() and v.dtype == self.cdtype
+        _check(_lib.hqmc_slab_scale(self._ctx, _ptr(v), C.c_longlong(v.numel()), C.c_double(s)))
+
+    def slab_sum_rows(self, rows, c0, c1, out):
+        """out[c0:c1] = sum over the rows (in order) of rows[:, c0:c1]; rows [k, m] and out [m]: device float64."""
+        assert rows.dim() == 2 and rows.is_contiguous() and rows.dtype == out.dtype == torch.float64 and 0 <= c0 < c1 <= rows.shape[1]
+        _check(_lib.hqmc_slab_sum_rows(self._ctx, C.c_void_p(rows.data_ptr() + 8 * c0), C.c_int(rows.shape[0]),
+                                       C.c_int(rows.shape[1]), C.c_int(c1 - c0), C.c_void_p(out.data_ptr() + 8 * c0)))
 
     # ---- host-buffer entry points (numpy arrays, pageable or pinned) ----------------------------
     def apply_MdagM_host(self, h_in: np.ndarray, h_out: np.ndarray):

@@ -1,0 +1,132 @@
+"""Host logic of the tau-slab path (paper_2508_16298_b200/slab.py) on CPU: the product's
+exchange / sign / range / sum logic driven with the oracle as the arithmetic (tests/slab_cpu_ops.py), in one process (several
+slabs per process) and over gloo with world_size 2, against the oracle's GLOBAL operators and PCG (Eq.8,
+:250-261 Eq.20, :316-326)."""
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2508_16298_b200 import inputs
+from paper_2508_16298_b200.slab import SlabLayout, SlabSolver
+from tests.slab_cpu_ops import OracleSlabOps
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def rel(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def parts(a, lay):
+    """The owned parts of a global array for the slabs of this process."""
+    return [torch.from_numpy(np.ascontiguousarray(a[lay.bounds[g]:lay.bounds[g + 1]])) for g in lay.owned]
+
+
+def gather(vs, lay, sol):
+    return np.concatenate([sol.own(v, i).numpy() for i, v in enumerate(vs)], axis=0)
+
+
+def test_layout_covers_the_lattice_once():
+    lay = SlabLayout(8, 26, 3, W=6)
+    assert [lay.nt(g) for g in range(3)] == [8, 9, 9] and lay.bounds[-1] == 26
+    assert lay.ext_slices(0)[:6] == [20, 21, 22, 23, 24, 25] and lay.ext_slices(2)[-6:] == [0, 1, 2, 3, 4, 5]
+    with pytest.raises(AssertionError):
+        SlabLayout(8, 10, 2, W=6)          # a slab shorter than the halo
+
+
+@pytest.mark.parametrize("S,W", [(1, 6), (2, 6), (3, 2), (4, 0)])
+def test_slab_operators_and_pcg_equal_the_global_ones(S, W):
+    L, Nt = 4, 26
+    theta = inputs.theta_uniform(L, Nt, 7)
+    v = inputs.complex_gaussian((Nt, L, L), 7)
+    o = orc.Oracle(L, Nt, W=W)
+    lay = SlabLayout(L, Nt, S, W=W)
+    ops = OracleSlabOps(lay)
+    sol = SlabSolver(lay, ops)
+    sol.set_theta(parts(theta, lay))
+    for g in lay.owned:                    # the extended theta of every slab is the global one at the extended slices
+        assert np.array_equal(sol.theta_ext[g].numpy(), theta[lay.ext_slices(g)])
+    vs = sol.extend(parts(v, lay), ops.new_vec)
+    outs = [ops.new_vec(i) for i in range(S)]
+    assert rel(gather(sol.apply_M(vs, outs), lay, sol), o.apply_M(theta, v)) <= 1e-14
+    assert rel(gather(sol.apply_Mdag(vs, outs), lay, sol), o.apply_Mdag(theta, v)) <= 1e-14
+    assert rel(gather(sol.apply_MdagM(vs, outs), lay, sol), o.apply_MdagM(theta, v)) <= 1e-14
+    if W:
+        assert rel(gather(sol.precond(vs, outs), lay, sol), o.precond(v)) <= 1e-14
+    fo = [ops.new_field(i) for i in range(S)]
+    ref = o.force_fermion(theta, v)
+    assert np.abs(gather(sol.force(vs, fo), lay, sol) - ref).max() <= 1e-13 * np.abs(ref).max()
+    phi = o.apply_Mdag(theta, v)
+    xs = [ops.new_vec(i) for i in range(S)]
+    it, relres, conv = sol.solve(sol.extend(parts(phi, lay), ops.new_vec), xs, 1e-10, 5000)
+    x_ref, it_ref, rel_ref = o.pcg(theta, phi, 1e-10, 5000)
+    assert conv and abs(it - it_ref) <= 2 and relres <= 1e-10
+    assert rel(gather(xs, lay, sol), x_ref) <= 1e-9
+    it, relres, conv = sol.solve(sol.extend(parts(phi, lay), ops.new_vec), xs, 0.0, 9)      # fixed count
+    x9, it9, rel9 = o.pcg(theta, phi, 0.0, 9)
+    assert it == it9 == 9 and rel(gather(xs, lay, sol), x9) <= 1e-12 and abs(relres - rel9) <= 1e-10 * rel9
+
+
+WORKER = r'''
+import os, sys
+sys.path.insert(0, sys.argv[1])
+import numpy as np, torch, torch.distributed as dist
+from oracle import oracle as orc
+from paper_2508_16298_b200 import inputs
+from paper_2508_16298_b200.slab import SlabLayout, SlabSolver
+from tests.slab_cpu_ops import OracleSlabOps
+rank, world, S = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"]), int(sys.argv[3])
+dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{sys.argv[2]}", rank=rank, world_size=world)
+orc.set_threads(1)
+L, Nt, W = 4, 30, 6
+theta = inputs.theta_uniform(L, Nt, 11)
+eta = inputs.complex_gaussian((Nt, L, L), 11)
+o = orc.Oracle(L, Nt, W=W)
+phi = o.apply_Mdag(theta, eta)
+lay = SlabLayout(L, Nt, S, W=W, world=world, rank=rank)
+ops = OracleSlabOps(lay)
+sol = SlabSolver(lay, ops)
+part = lambda a: [torch.from_numpy(np.ascontiguousarray(a[lay.bounds[g]:lay.bounds[g + 1]])) for g in lay.owned]
+sol.set_theta(part(theta))                              # every rank passes ONLY its own slices; halos arrive over gloo
+vs = sol.extend(part(eta), ops.new_vec)
+outs = [ops.new_vec(i) for i in range(len(lay.owned))]
+sol.apply_MdagM(vs, outs)
+ref = o.apply_MdagM(theta, eta)
+e_op = max(float(np.abs(sol.own(outs[i], i).numpy() - ref[lay.bounds[g]:lay.bounds[g + 1]]).max()) for i, g in enumerate(lay.owned))
+xs = [ops.new_vec(i) for i in range(len(lay.owned))]
+it, relres, conv = sol.solve(sol.extend(part(phi), ops.new_vec), xs, 1e-10, 5000)
+x_ref, it_ref, _ = o.pcg(theta, phi, 1e-10, 5000)
+e_x = max(float(np.abs(sol.own(xs[i], i).numpy() - x_ref[lay.bounds[g]:lay.bounds[g + 1]]).max()) for i, g in enumerate(lay.owned))
+dist.barrier()
+print(f"RESULT {rank} {e_op / np.abs(ref).max():.3e} {e_x / np.abs(x_ref).max():.3e} {it} {it_ref} {int(conv)}")
+dist.destroy_process_group()
+'''
+
+
+@pytest.mark.parametrize("S", [2, 4])
+def test_slab_pcg_gloo_world2(tmp_path, S):
+    """N>1 path: two processes, one or two slabs each, halos and sums over gloo; every rank's slices of M^+M v and of the PCG
+    solution equal the oracle's global result."""
+    script = tmp_path / "slab_worker.py"
+    script.write_text(WORKER)
+    port = 29600 + (os.getpid() % 300) + S
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), OMP_NUM_THREADS="1")
+        procs.append(subprocess.Popen([sys.executable, str(script), ROOT, str(port), str(S)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=300) for p in procs]
+    assert all(p.returncode == 0 for p in procs), outs
+    seen = 0
+    for out, _ in outs:
+        for line in out.splitlines():
+            if line.startswith("RESULT"):
+                _, rank, e_op, e_x, it, it_ref, conv = line.split()
+                assert float(e_op) <= 1e-14 and float(e_x) <= 1e-9 and abs(int(it) - int(it_ref)) <= 2 and conv == "1"
+                seen += 1
+    assert seen == 2
