@@ -404,9 +404,17 @@ def contract_numbers(args, torch, hqmc, inputs, theta_cfg, eta_cfg):
         Ng = 10 * Lg
         th, p0 = inputs.theta_uniform(Lg, Ng, 7), inputs.momenta(Lg, Ng, 7)
         res, fin = {}, {}
-        for on in (True, False):
+        for on in (True, False, "persistent"):
             g = hqmc.HQMC(Lg, Ng)
-            g.set_md_graph(on)
+            if on == "persistent":                      # the whole solve as one persistent kernel (small lattices only)
+                try:
+                    g.set_cg_persistent(hqmc.PERSIST_ON)
+                except hqmc.HqmcError:
+                    g.close()
+                    continue
+            else:
+                g.set_cg_persistent(hqmc.PERSIST_OFF)
+                g.set_md_graph(on)
             g.set_theta(dev(th))
             phi = g.apply_Mdag(dev(inputs.complex_gaussian((Ng, Lg, Lg), 7)))
             best = 1e30
@@ -417,12 +425,34 @@ def contract_numbers(args, torch, hqmc, inputs, theta_cfg, eta_cfg):
                 e0.record(); g.trajectory(d_th, d_p, phi, 3, 0.01, cg_tol=0.0, cg_max_iter=100); e1.record(); torch.cuda.synchronize()
                 if k:
                     best = min(best, e0.elapsed_time(e1))
-            res["graph" if on else "plain"] = best
+            res[on if on == "persistent" else ("graph" if on else "plain")] = best
             fin[on] = (d_th, d_p)
             g.close()
         mg[f"L{Lg}"] = {"ms_graph": res["graph"], "ms_plain": res["plain"], "speedup": res["plain"] / res["graph"],
                         "bitwise_identical": bool(torch.equal(fin[True][0], fin[False][0]) and torch.equal(fin[True][1], fin[False][1]))}
+        if "persistent" in res:
+            mg[f"L{Lg}"]["ms_persistent_kernel"] = res["persistent"]
+            mg[f"L{Lg}"]["max_abs_diff_theta_persistent"] = float((fin["persistent"][0] - fin[True][0]).abs().max())
     out["md_graph"] = mg
+    # one chain of a small lattice (PAPER.md:350's launch-bound regime): the four-kernel graph-replayed loop against the
+    # one-launch persistent kernel (pcg_persist.cuh), us per PCG iteration over 2000 fixed iterations
+    pp = {"protocol": "uniform theta, Ntau = 10 L, 2000 fixed iterations, wall clock around hqmc_cg_solve; us per iteration"}
+    for Lp in (8, 12, 16, 20):
+        Np = 10 * Lp
+        g = hqmc.HQMC(Lp, Np)
+        g.set_theta(dev(inputs.theta_uniform(Lp, Np, 7)))
+        phi = g.apply_Mdag(dev(inputs.complex_gaussian((Np, Lp, Lp), 7)))
+        row = {}
+        for name, mode in (("loop", hqmc.PERSIST_OFF), ("persistent", hqmc.PERSIST_ON)):
+            g.set_cg_persistent(mode)
+            g.cg_solve(phi, 0.0, 200)
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            g.cg_solve(phi, 0.0, 2000)
+            torch.cuda.synchronize()
+            row[name] = 1e6 * (time.perf_counter() - t0) / 2000
+        pp[f"L{Lp}"] = row
+        g.close()
+    out["pcg_persistent"] = pp
     return out
 
 

@@ -43,6 +43,18 @@ int hqmc_set_precond_tile(hqmc_ctx *ctx, int slices_per_run);
 enum { HQMC_CG_AUTO = 0, HQMC_CG_TEXTBOOK = 1, HQMC_CG_DEFERRED_X = 2 };
 int hqmc_set_cg_variant(hqmc_ctx *ctx, int which);
 
+/* Whole PCG solve as ONE persistent cooperative kernel (pcg_persist.cuh; small lattices are launch-bound):
+ * one CTA per time slice, x, r, d, z and the decoded links in registers for the whole solve; per iteration the two global sums
+ * of Eq.20 as all-to-all exchanges of tagged words and two point-to-point halo hand-overs, no kernel boundary, no atomic.
+ * Usable where one thread holds a 2x2 block and all Ntau CTAs are resident at once (L <= 22 at Ntau = 10 L on a B200).  AUTO
+ * (default) = taken by hqmc_cg_solve and every entry point that solves to a tolerance through it (trajectories, sweeps, the
+ * one-vector path of hqmc_green_apply) where usable and the lattice has at most HQMC_PERSIST_AUTO_SITES sites (measured: 10.8 us
+ * per iteration against 15.5-17.3 for the four-kernel graph at L = 8...16, 15.5 against 18.9 at L = 20); OFF = never; ON = wherever
+ * usable (HQMC_EINVAL where it is not).  Same iterates as the four-kernel loop up to the order of the sums. */
+enum { HQMC_PERSIST_AUTO = 0, HQMC_PERSIST_OFF = 1, HQMC_PERSIST_ON = 2 };
+#define HQMC_PERSIST_AUTO_SITES 100000
+int hqmc_set_cg_persistent(hqmc_ctx *ctx, int mode);
+
 /* Vectors hqmc_green_apply solves per launch: 0 (default) = as many as keep the batch's live set L2-resident, 1 = one
  * at a time on the one-vector kernels, n > 1 = n at a time. */
 int hqmc_set_green_batch(hqmc_ctx *ctx, int n);

@@ -84,8 +84,40 @@ template <typename T> static int cg_enqueue_fixed(hqmc_ctx *c, const void *rhs, 
     return HQMC_OK;
 }
 
+// Small lattices (PAPER.md:350's launch-bound regime): the whole solve is ONE cooperative launch of k_pcg_persist.  AUTO takes it
+// where an iteration of the four-kernel loop is all launch and drain (measured: profiles/r02_summary.md section 6).
+static bool cg_use_persistent(const hqmc_ctx *c) {
+    if (!c->persist_ok || c->persist_mode == 1 || c->profiling || c->skip_mask) return false;
+    return c->persist_mode == 2 || c->N <= HQMC_PERSIST_AUTO_SITES;
+}
+template <typename T> static int cg_solve_persistent(hqmc_ctx *c, const void *rhs, void *x, double tol, long long max_iter) {
+    typedef typename Cx<T>::type T2;
+    CUDA_TRY(cudaMemsetAsync(c->d_ctr, 0, sizeof(unsigned long long) * HQMC_SYNC_WORDS(c->g.Nt), c->stream));
+    Geo g = c->g; Taps taps = c->taps; T C = (T)c->C;
+    const T2 *ph = (const T2 *)c->d_ph, *b = (const T2 *)rhs;
+    T2 *xx = (T2 *)x, *rb = (T2 *)c->d_r, *db = (T2 *)c->d_d;
+    double tol2 = tol > 0.0 ? tol * tol : 0.0;
+    unsigned long long *ctr = c->d_ctr; CgState *st = c->d_state;
+    void *args[] = {&g, &taps, &ph, &b, &xx, &rb, &db, &C, &ctr, &st, &tol2, &max_iter};
+    const void *fn = (const void *)k_pcg_persist<T>;
+    CUDA_TRY(cudaLaunchCooperativeKernel(fn, dim3(c->g.Nt), dim3(c->cfg.threads), args, c->persist_smem, c->stream));
+    c->launches[HQMC_K_MISC]++;
+    return HQMC_OK;
+}
+
 template <typename T> static int cg_solve_t(hqmc_ctx *c, const void *rhs, void *x, double tol, long long max_iter,
                                             long long *iters_out, double *relres_out) {
+    if (cg_use_persistent(c)) {
+        HQ_TRY(cg_solve_persistent<T>(c, rhs, x, tol, max_iter));
+        CUDA_TRY(cudaMemcpyAsync(c->h_state, c->d_state, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(cudaStreamSynchronize(c->stream));
+        const double bb = c->h_state->bb, rr = c->h_state->rr;
+        const double rel = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
+        if (iters_out) *iters_out = c->h_state->iters;
+        if (relres_out) *relres_out = rel;
+        if (rel != rel || (tol > 0.0 && !(rel <= tol))) return HQMC_ENOCONV;
+        return HQMC_OK;
+    }
     HQ_TRY(cg_start<T>(c, rhs, x, tol, max_iter));
     const bool use_graph = !c->profiling;
     if (use_graph) HQ_TRY(cg_build_graph<T>(c, x));

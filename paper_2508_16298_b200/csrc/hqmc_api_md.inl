@@ -92,6 +92,10 @@ extern "C" int hqmc_leapfrog_trajectory(hqmc_ctx *c, double *d_theta, double *d_
     long long total = 0, it = 0;
     bool noconv = false;
     auto solve = [&]() -> int {
+        if (cg_tol <= 0.0 && cg_use_persistent(c)) {                        // fixed count on a small lattice: one launch, no host round trip
+            total += cg_max_iter;
+            return DISPATCH_T(c, cg_solve_persistent<double>(c, d_pf, c->d_X, 0.0, cg_max_iter), cg_solve_persistent<float>(c, d_pf, c->d_X, 0.0, cg_max_iter));
+        }
         int s = cg_solve_any(c, d_pf, c->d_X, cg_tol, cg_max_iter, &it, nullptr);
         total += it;
         if (s == HQMC_ENOCONV) { noconv = true; return HQMC_OK; }
@@ -101,7 +105,8 @@ extern "C" int hqmc_leapfrog_trajectory(hqmc_ctx *c, double *d_theta, double *d_
     CUDA_TRY(cudaMemsetAsync(c->d_scal, 0, sizeof(double) * 8, c->stream));
     HQ_TRY(solve());
     HQ_TRY(enqueue_energies(c, d_p, d_pf, c->d_X, 0));                      // H0 parts -> d_scal[0..2]
-    bool step_graph = c->md_graph && !c->md_graph_broken && !c->profiling && c->skip_mask == 0 && cg_tol <= 0.0 && cg_max_iter > 0;
+    bool step_graph = c->md_graph && !c->md_graph_broken && !c->profiling && c->skip_mask == 0 && cg_tol <= 0.0 && cg_max_iter > 0 &&
+                      !cg_use_persistent(c);        // (the persistent solve is already one launch)
     for (int n = 0; n < nsteps; ++n) {
         if (n == 0) HQ_TRY(kick(c, d_p, 0.5 * eps, 1));                     // p += F(theta_0) eps/2
         if (step_graph) {

@@ -146,6 +146,18 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     st = build_default_taps(c);
     if (st != HQMC_OK) return fail(st);
     precond_cfg(c, 0);
+    {   // persistent whole-solve kernel: one CTA per slice, all of them resident at once (cooperative launch)
+        int coop = 0, per_sm = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        c->persist_smem = block_smem(c) + 8 * sizeof(double);
+        if (coop && c->cfg.bpt == 1 && c->cfg.threads <= 256 && c->g.Nt <= 8 * c->cfg.threads) {
+            const void *fn = (prm->prec == HQMC_C128) ? (const void *)k_pcg_persist<double> : (const void *)k_pcg_persist<float>;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, c->cfg.threads, c->persist_smem);
+            if (e != cudaSuccess) { per_sm = 0; cudaGetLastError(); }
+            c->persist_ok = (long long)per_sm * c->n_sm >= c->g.Nt;
+        }
+        if (c->persist_ok && cudaMalloc((void **)&c->d_ctr, sizeof(unsigned long long) * HQMC_SYNC_WORDS(c->g.Nt)) != cudaSuccess) { cudaGetLastError(); c->persist_ok = false; }
+    }
     *out = c;
     return HQMC_OK;
 }
@@ -163,7 +175,7 @@ extern "C" int hqmc_destroy(hqmc_ctx *c) {
     for (auto &ep : c->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     if (c->ms_plan_ok) cufftDestroy(c->ms_plan);
     void *ptrs[] = {c->d_ms_a, c->d_ms_b, c->d_ms_acc, c->d_packed, c->d_tab, c->d_theta, c->d_ph, c->d_r, c->d_z, c->d_d, c->d_Od, c->d_X, c->d_phi, c->d_p, c->d_force, c->d_part_dOd,
-                    c->d_part_rr, c->d_part_rz[0], c->d_part_rz[1], c->d_part_misc, c->d_state, c->d_scal};
+                    c->d_part_rr, c->d_part_rz[0], c->d_part_rz[1], c->d_part_misc, c->d_state, c->d_scal, c->d_ctr};
     for (void *p : ptrs) if (p) cudaFree(p);
     if (c->h_state) cudaFreeHost(c->h_state);
     if (c->h_scal) cudaFreeHost(c->h_scal);
@@ -276,6 +288,13 @@ extern "C" int hqmc_set_md_graph(hqmc_ctx *c, int on) {
     c->md_graph = on != 0;
     return HQMC_OK;
 }
+extern "C" int hqmc_set_cg_persistent(hqmc_ctx *c, int mode) {
+    if (!c || mode < 0 || mode > 2) return HQMC_EINVAL;
+    if (mode == HQMC_PERSIST_ON && !c->persist_ok) { g_last_error = "the persistent PCG kernel cannot run this lattice (one 2x2 block per thread, all Ntau CTAs resident)"; return HQMC_EINVAL; }
+    c->persist_mode = mode;
+    return HQMC_OK;
+}
+
 extern "C" int hqmc_set_cg_variant(hqmc_ctx *c, int which) {
     if (!c || which < HQMC_CG_AUTO || which > HQMC_CG_DEFERRED_X) return HQMC_EINVAL;
     c->cg_defer_x = which == HQMC_CG_DEFERRED_X || (which == HQMC_CG_AUTO && cg_defer_default(c));

@@ -24,6 +24,7 @@
 #include "cg_batched.cuh"
 #include "rng_kernels.cuh"
 #include "slab_kernels.cuh"
+#include "pcg_persist.cuh"
 
 namespace hqmc {
 
@@ -114,6 +115,9 @@ struct hqmc_ctx {
     void *cgb_graph_x = nullptr; int cgb_graph_n = 0, cgb_graph_tt = 0, cgb_graph_W = -1;
     long long cgb_nodes[HQMC_K_COUNT] = {};
     int green_batch = 0;                   // hqmc_set_green_batch: 0 = by footprint, 1 = one vector at a time, n = n at a time
+    // whole-solve persistent kernel (pcg_persist.cuh): usable (one block per thread, all Ntau CTAs co-resident) / mode
+    bool persist_ok = false; int persist_mode = 0;        // 0 = auto (small lattices), 1 = never, 2 = whenever usable
+    size_t persist_smem = 0; unsigned long long *d_ctr = nullptr;
     bool cg_defer_x;     // deferred-x PCG vector kernels (k_cg_raxpy + k_cg_xdupdate)
     int cg_chunk;            // iterations per graph launch
     bool md_graph = true;    // leapfrog steps with fixed-count solves replayed as one CUDA graph (hqmc_set_md_graph)

@@ -19,6 +19,7 @@ HQMC_OK, HQMC_EINVAL, HQMC_ECUDA, HQMC_ENOCONV, HQMC_ENOMEM = 0, -1, -2, -3, -4
 K_MDAGM, K_AXPY, K_PRECOND, K_DUPDATE, K_M, K_FORCE, K_PHASE, K_MISC, K_COUNT = range(9)
 MDAGM_AUTO, MDAGM_REGISTER, MDAGM_CLUSTER, MDAGM_STREAM = 0, 1, 2, 3
 CG_AUTO, CG_TEXTBOOK, CG_DEFERRED_X = 0, 1, 2
+PERSIST_AUTO, PERSIST_OFF, PERSIST_ON = 0, 1, 2
 KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force", "phase", "misc"]
 
 # every symbol include/hqmc.h and include/hqmc_tuning.h declare
@@ -29,7 +30,7 @@ SYMBOLS = [
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_action_boson_noalloc", "hqmc_slab_dot", "hqmc_slab_axpy", "hqmc_slab_dupdate",
     "hqmc_slab_scale", "hqmc_slab_sum_rows", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
-    "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_variant", "hqmc_set_md_graph", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
+    "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_variant", "hqmc_set_cg_persistent", "hqmc_set_md_graph", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
 
 
@@ -134,6 +135,10 @@ class HQMC:
     def set_cg_variant(self, which: int):
         """CG_AUTO / CG_TEXTBOOK / CG_DEFERRED_X (include/hqmc_tuning.h)."""
         _check(_lib.hqmc_set_cg_variant(self._ctx, C.c_int(int(which))))
+
+    def set_cg_persistent(self, mode: int):
+        """PERSIST_AUTO / PERSIST_OFF / PERSIST_ON: the whole-solve persistent kernel (include/hqmc_tuning.h)."""
+        _check(_lib.hqmc_set_cg_persistent(self._ctx, C.c_int(int(mode))))
 
     def set_md_graph(self, on: bool):
         _check(_lib.hqmc_set_md_graph(self._ctx, C.c_int(int(on))))

@@ -205,6 +205,38 @@ def test_leapfrog_step_graph_is_bitwise_identical_to_plain_launches(hq, L, Nt):
     assert out[0][2:] == out[1][2:] and out[0][4] == 70 * 5
 
 
+def test_persistent_pcg_kernel_selection_and_limits(hq):
+    """include/hqmc_tuning.h hqmc_set_cg_persistent: AUTO takes the one-launch kernel on small lattices (bitwise the same as
+    ON, one launch instead of four per iteration), refuses lattices it cannot hold, complex64 runs through it too."""
+    L, Nt = 12, 120
+    theta = inputs.theta_uniform(L, Nt, 8)
+    phi = inputs.complex_gaussian((Nt, L, L), 8)
+    g = hq.HQMC(L, Nt)
+    g.set_theta(dev(theta))
+    out = {}
+    for mode in (hq.PERSIST_AUTO, hq.PERSIST_ON, hq.PERSIST_OFF):
+        g.set_cg_persistent(mode)
+        g.reset_stats()
+        x, it, relres, _ = g.cg_solve(dev(phi), 0.0, 30)
+        out[mode] = (x.clone(), relres, sum(v[0] for v in g.kernel_stats().values()))
+    assert torch.equal(out[hq.PERSIST_AUTO][0], out[hq.PERSIST_ON][0]) and out[hq.PERSIST_AUTO][2] == 1
+    assert out[hq.PERSIST_OFF][2] >= 4 * 30
+    assert rel(out[hq.PERSIST_ON][0].cpu().numpy(), out[hq.PERSIST_OFF][0].cpu().numpy()) <= 1e-12
+    g.close()
+    big = hq.HQMC(48, 20)
+    with pytest.raises(hq.HqmcError):
+        big.set_cg_persistent(hq.PERSIST_ON)
+    big.close()
+    o = orc.Oracle(L, Nt)
+    g = hq.HQMC(L, Nt, prec="c64")
+    g.set_theta(dev(theta))
+    g.set_cg_persistent(hq.PERSIST_ON)
+    x, it, relres, _ = g.cg_solve(dev(phi.astype(np.complex64)), 0.0, 12)
+    xo, _, relo = o.pcg(theta, phi, 0.0, 12)
+    assert it == 12 and np.linalg.norm(x.cpu().numpy().astype(np.complex128).ravel() - xo.ravel()) / np.linalg.norm(xo.ravel()) <= 1e-5
+    g.close()
+
+
 def test_device_random_numbers_match_the_cpu_twin_bit_for_bit(hq):
     """NEXT-1 (reading C25): same (seed, update, stream, element) -> the same Philox4x32-10 words bit
     for bit, hence the same 53-bit uniforms; the Gaussians differ only by the last bits of log / sincos."""

@@ -89,9 +89,12 @@ def test_precond_and_taps(hq, L, Nt, W):
     g.close()
 
 
-@pytest.mark.parametrize("L,Nt,seed,W", [(4, 8, 0, 6), (4, 8, 0, 0), (6, 10, 1, 6), (8, 40, 2, 6), (8, 40, 2, 10)])
-def test_cg_solution_and_iterations(hq, L, Nt, seed, W):
+@pytest.mark.parametrize("persistent", [False, True])
+@pytest.mark.parametrize("L,Nt,seed,W", [(4, 8, 0, 6), (4, 8, 0, 0), (6, 10, 1, 6), (8, 40, 2, 6), (8, 40, 2, 10), (14, 50, 3, 6), (20, 200, 4, 6)])
+def test_cg_solution_and_iterations(hq, L, Nt, seed, W, persistent):
+    """The PCG of Eq.20 as the four-kernel graph-replayed loop and as the one-launch persistent kernel (pcg_persist.cuh)."""
     o, g, theta = setup(hq, L, Nt, seed, W=W)
+    g.set_cg_persistent(hq.PERSIST_ON if persistent else hq.PERSIST_OFF)
     eta = inputs.complex_gaussian((Nt, L, L), seed)
     phi = o.apply_Mdag(theta, eta)
     x_ref, it_ref, rel_ref = o.pcg(theta, phi, 1e-10, 100000)
@@ -123,6 +126,7 @@ def test_cg_solution_and_iterations(hq, L, Nt, seed, W):
 def test_cg_variants_agree_with_oracle(hq, L, Nt, seed, W):
     """Default, deferred-x and textbook PCG vector kernels all give the oracle's iterates."""
     o, g, theta = setup(hq, L, Nt, seed, W=W)
+    g.set_cg_persistent(hq.PERSIST_OFF)          # the vector kernels of the four-kernel loop are what is tested here
     eta = inputs.complex_gaussian((Nt, L, L), seed)
     phi = o.apply_Mdag(theta, eta)
     xo, ito, relo = o.pcg(theta, phi, 0.0, 25)
@@ -255,6 +259,11 @@ def test_kernels_are_deterministic_run_to_run(hq, L, Nt):
             g.apply_MdagM(v, out)
             assert torch.equal(out, ref), (which, rep)
     g.set_mdagm_kernel(hq.MDAGM_AUTO)
+    if L <= 16:                                  # the persistent whole-solve kernel: tagged-word exchanges, no atomics
+        g.set_cg_persistent(hq.PERSIST_ON)
+        xs = [g.cg_solve(v, 0.0, 64)[0].clone() for _ in range(5)]
+        assert all(torch.equal(xs[0], x) for x in xs[1:])
+    g.set_cg_persistent(hq.PERSIST_OFF)
     for fused in (hq.CG_AUTO, hq.CG_DEFERRED_X, hq.CG_TEXTBOOK):
         g.set_cg_variant(fused)
         x1 = g.cg_solve(v, 0.0, 64)[0].clone()
