@@ -108,7 +108,12 @@ template <typename T> static int cg_solve_persistent(hqmc_ctx *c, const void *rh
 template <typename T> static int cg_solve_t(hqmc_ctx *c, const void *rhs, void *x, double tol, long long max_iter,
                                             long long *iters_out, double *relres_out) {
     if (cg_use_persistent(c)) {
-        HQ_TRY(cg_solve_persistent<T>(c, rhs, x, tol, max_iter));
+        const int sp = cg_solve_persistent<T>(c, rhs, x, tol, max_iter);
+        if (sp != HQMC_OK) {      // the cooperative launch was refused (e.g. the device is shared): the four-kernel loop from now on
+            cudaGetLastError();
+            c->persist_ok = false;
+            return cg_solve_t<T>(c, rhs, x, tol, max_iter, iters_out, relres_out);
+        }
         CUDA_TRY(cudaMemcpyAsync(c->h_state, c->d_state, sizeof(CgState), cudaMemcpyDeviceToHost, c->stream));
         CUDA_TRY(cudaStreamSynchronize(c->stream));
         const double bb = c->h_state->bb, rr = c->h_state->rr;

@@ -122,6 +122,29 @@ def test_cg_solution_and_iterations(hq, L, Nt, seed, W, persistent):
     g.close()
 
 
+@pytest.mark.parametrize("persistent", [False, True])
+@pytest.mark.parametrize("L,Nt,W", [(4, 2, 1), (4, 2, 0), (4, 3, 2), (6, 7, 6), (10, 5, 4)])
+def test_cg_on_degenerate_time_extents(hq, L, Nt, W, persistent):
+    """The shortest lattices the library accepts (Ntau = 2: both neighbours of a slice are the same slice, every tap wraps),
+    taps reaching all the way round (2 W + 1 > Ntau), an odd number of slices: both PCG forms against the oracle."""
+    o, g, theta = setup(hq, L, Nt, 9, W=W)
+    g.set_cg_persistent(hq.PERSIST_ON if persistent else hq.PERSIST_OFF)
+    eta = inputs.complex_gaussian((Nt, L, L), 9)
+    phi = o.apply_Mdag(theta, eta)
+    assert rel(g.apply_MdagM(dev(eta)).cpu().numpy(), o.apply_MdagM(theta, eta)) <= 1e-12
+    if W:
+        assert rel(g.precond(dev(eta)).cpu().numpy(), o.precond(eta)) <= 1e-13
+    x_ref, it_ref, _ = o.pcg(theta, phi, 1e-10, 10000)
+    x, it, relres, ok = g.cg_solve(dev(phi), 1e-10, 10000)
+    assert ok and relres <= 1e-10 and abs(it - it_ref) <= 2 and rel(x.cpu().numpy(), x_ref) <= 1e-9
+    xf, itf, relf, _ = g.cg_solve(dev(phi), 0.0, 5)
+    xo, ito, relo = o.pcg(theta, phi, 0.0, 5)
+    assert itf == ito == 5 and rel(xf.cpu().numpy(), xo) <= 1e-11 and abs(relf - relo) <= 1e-9 * relo
+    x0, it0, rel0, _ = g.cg_solve(dev(phi), 0.0, 0)              # no iteration at all: x = 0, the residual is the right-hand side
+    assert it0 == 0 and float(x0.abs().max()) == 0.0 and abs(rel0 - 1.0) <= 1e-15
+    g.close()
+
+
 @pytest.mark.parametrize("L,Nt,seed,W", [(8, 40, 2, 6), (12, 30, 3, 3), (6, 10, 1, 1)])
 def test_cg_variants_agree_with_oracle(hq, L, Nt, seed, W):
     """Default, deferred-x and textbook PCG vector kernels all give the oracle's iterates."""
