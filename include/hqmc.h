@@ -3,7 +3,7 @@
  * method of arxiv/paper_2508_16298 ("Scalable hybrid quantum Monte Carlo simulation of U(1) gauge
  * field coupled to fermions on GPU"), hand-written CUDA for sm_100a (NVIDIA B200).
  *
- * Citations are to /root/reference/PAPER.md (line numbers) and to the readings C1-C24 listed in
+ * Citations are to /root/reference/PAPER.md (line numbers) and to the readings C1-C25 listed in
  * DESIGN.md (taken from SURVEY.md section 8c).
  *
  * Conventions (all entry points)
@@ -220,6 +220,13 @@ int hqmc_slab_dupdate(hqmc_ctx *ctx, void *d_d, const void *d_z, long long n, co
 int hqmc_slab_scale(hqmc_ctx *ctx, void *d_v, long long n, double s);
 /* d_out[j] = sum_i d_in[i * stride + j], i < rows in order, j < cols: the partial sums of the slabs one process owns. */
 int hqmc_slab_sum_rows(hqmc_ctx *ctx, const double *d_in, int rows, int stride, int cols, double *d_out);
+/* y += a x over n doubles: the drift theta += 2 eps p and the kicks p -= (eps/2) dS/dtheta on a slab's owned slices
+ * (Eq.16; dS_F/dtheta from hqmc_force, dS_B/dtheta from hqmc_force_boson of the extended context). */
+int hqmc_slab_field_axpy(hqmc_ctx *ctx, double *d_y, const double *d_x, double a, long long n);
+/* d_out[0] = the part of S_B that belongs to the slices [first_slice, first_slice + n_slices) of the context's
+ * (extended) theta: their plaquette terms and the temporal terms between slice t and t + 1, no wrap -- slice
+ * first_slice + n_slices must exist (the upper halo), else HQMC_EINVAL.  Summed over the slabs it is the global S_B. */
+int hqmc_slab_action_boson(hqmc_ctx *ctx, int first_slice, int n_slices, double *d_out);
 
 /* HOST-buffer variants (pageable or pinned host memory; the copies run inside the call on the
  * context's stream and the call returns after the result has landed in h_out / h_x). */

@@ -54,3 +54,18 @@ extern "C" int hqmc_slab_sum_rows(hqmc_ctx *c, const double *d_in, int rows, int
     if (!c || !d_in || !d_out || rows < 1 || cols < 1 || stride < cols) return HQMC_EINVAL;
     return launch(c, HQMC_K_MISC, k_slab_sum_rows, dim3((cols + 63) / 64), dim3(64), 0, d_in, rows, stride, cols, d_out);
 }
+
+extern "C" int hqmc_slab_field_axpy(hqmc_ctx *c, double *d_y, const double *d_x, double a, long long n) {
+    if (!c || n < 0 || !d_y || !d_x) return HQMC_EINVAL;
+    if (n == 0) return HQMC_OK;
+    return launch(c, HQMC_K_MISC, k_slab_field_axpy, dim3(slab_grid(c, n)), dim3(256), 0, (size_t)n, d_y, d_x, a);
+}
+
+extern "C" int hqmc_slab_action_boson(hqmc_ctx *c, int first_slice, int n_slices, double *d_out) {
+    if (!c || !d_out || first_slice < 0 || n_slices < 1 || first_slice + n_slices >= c->g.Nt) return HQMC_EINVAL;
+    if (!c->theta_set) { g_last_error = "hqmc_set_theta has not been called"; return HQMC_EINVAL; }
+    const int G = slab_grid(c, (long long)2 * c->g.Vs * n_slices);
+    HQ_TRY(launch(c, HQMC_K_MISC, k_slab_action_boson, dim3(G), dim3(256), 0, c->g, (const double *)c->d_theta, first_slice, n_slices,
+                  c->prm.c_tau, c->prm.K, c->prm.compact, c->d_part_misc));
+    return launch(c, HQMC_K_MISC, k_final_sum, dim3(1), dim3(32), 0, (const double *)c->d_part_misc, G, d_out);
+}

@@ -9,6 +9,7 @@
 // Sums are two-stage and run in a fixed order (one partial per CTA, then k_final_sum): deterministic run to run.
 #pragma once
 #include "cg_kernels.cuh"
+#include "force_kernels.cuh"
 
 namespace hqmc {
 
@@ -53,6 +54,32 @@ __global__ void k_slab_scale(size_t n, typename Cx<T>::type *__restrict__ v, T s
         a.x *= s; a.y *= s;
         v[i] = a;
     }
+}
+
+// y += a x over n doubles: the drift theta += 2 eps p and the kicks p -= (eps/2) dS/dtheta of a slab's owned slices (Eq.16)
+__global__ void k_slab_field_axpy(size_t n, double *__restrict__ y, const double *__restrict__ x, double a) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) y[i] = fma(a, x[i], y[i]);
+}
+
+// S_B restricted to the slices [first, first + count) of an extended lattice: the temporal term of slice t couples
+// it to slice t + 1, which must exist in the buffer (the upper halo); no wrap.  One partial per CTA.
+__global__ void k_slab_action_boson(Geo g, const double *__restrict__ theta, int first, int count, double c_tau, double K, int compact,
+                                    double *__restrict__ part) {
+    __shared__ double red[32];
+    const size_t per = (size_t)2 * g.Vs, n = per * (size_t)count;
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int t = first + (int)(i / per);
+        const int r = (int)(i % per);
+        const double d = theta[(size_t)(t + 1) * per + r] - theta[(size_t)t * per + r];
+        acc += c_tau * (compact ? (1.0 - cos(d)) : d * d);
+        if (r < g.Vs) {
+            const int y = r / g.L, x = r - y * g.L;
+            acc += K * cos(curl_at(theta + (size_t)t * per, g.L, g.Vs, x, y));
+        }
+    }
+    const double s = block_sum(acc, red);
+    if (threadIdx.x == 0) part[blockIdx.x] = s;
 }
 
 // out[j] = sum_{i < rows} in[i * stride + j], j < cols, rows added in index order (the slabs one process owns)

@@ -29,7 +29,7 @@ SYMBOLS = [
     "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_rng_raw", "hqmc_rng_gauss", "hqmc_rng_uniform", "hqmc_sweep", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_action_boson_noalloc", "hqmc_slab_dot", "hqmc_slab_axpy", "hqmc_slab_dupdate",
-    "hqmc_slab_scale", "hqmc_slab_sum_rows", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
+    "hqmc_slab_scale", "hqmc_slab_sum_rows", "hqmc_slab_field_axpy", "hqmc_slab_action_boson", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
     "hqmc_set_time_tile", "hqmc_set_mdagm_kernel", "hqmc_set_precond_tile", "hqmc_set_cg_variant", "hqmc_set_cg_persistent", "hqmc_set_md_graph", "hqmc_set_pdl", "hqmc_set_debug_skip", "hqmc_strerror", "hqmc_last_error", "hqmc_version",
 ]
 
@@ -340,6 +340,15 @@ class HQMC:
     def slab_scale(self, v, s):
         assert v.is_contiguous() and v.dtype == self.cdtype
         _check(_lib.hqmc_slab_scale(self._ctx, _ptr(v), C.c_longlong(v.numel()), C.c_double(s)))
+
+    def slab_field_axpy(self, y, x, a):
+        """y += a x on float64 views (drift and kicks of a slab's owned slices)."""
+        assert y.is_contiguous() and x.is_contiguous() and y.dtype == x.dtype == torch.float64 and y.numel() == x.numel()
+        _check(_lib.hqmc_slab_field_axpy(self._ctx, _ptr(y), _ptr(x), C.c_double(a), C.c_longlong(y.numel())))
+
+    def slab_action_boson(self, first_slice, n_slices, out):
+        """out[0] = the share of S_B of slices [first_slice, first_slice + n_slices) of the context's theta."""
+        _check(_lib.hqmc_slab_action_boson(self._ctx, C.c_int(first_slice), C.c_int(n_slices), _ptr(out)))
 
     def slab_sum_rows(self, rows, c0, c1, out):
         """out[c0:c1] = sum over the rows (in order) of rows[:, c0:c1]; rows [k, m] and out [m]: device float64."""

@@ -160,6 +160,21 @@ class CudaSlabOps:
     def force(self, i, x, out):
         self.ctx[i].force(x, out)
 
+    def force_boson(self, i, out):
+        self.ctx[i].force_boson(out)
+
+    def field_axpy(self, i, y, x, a):
+        self.ctx[i].slab_field_axpy(y, x, a)
+
+    def action_boson(self, i, first, count, out):
+        self.ctx[i].slab_action_boson(first, count, out)
+
+    def sum_squares(self, i, f, out):
+        """out[0] = sum of f^2 over a float64 view (its pairs of doubles read as complex numbers: Re <f, f>)."""
+        assert self.cdtype == torch.complex128, "the slab trajectory runs in complex128"
+        v = torch.view_as_complex(f.reshape(-1, 2))
+        self.ctx[i].slab_dot(v, v, out)
+
     def dot(self, i, a, b, out):
         self.ctx[i].slab_dot(a, b, out)
 
@@ -354,3 +369,60 @@ class SlabSolver:
             last = RR1 if (it & 1) == 1 else RR0
             rel = (float(s[last]) / float(s[BB])) ** 0.5 if float(s[BB]) > 0 else 0.0
         return it, rel, conv
+
+
+    # ---- molecular dynamics on the sharded lattice (PAPER.md:207-214 Eq.16, :181 Eq.12; reading C7) -----------------------
+    def energies(self, p_own, phi, x):
+        """H = S_B + sum p^2 + Re <phi, x>, every term summed over the owned slices of every slab, then over the processes."""
+        lay, ops = self.lay, self.ops
+        if not hasattr(self, "_erows"):
+            self._erows, self._es = ops.scalars(self.k, 3), ops.scalars(3)
+        with self._stream():
+            for i, g in enumerate(lay.owned):
+                ops.action_boson(i, lay.H, lay.nt(g), self._erows[i, 0:1])
+                ops.sum_squares(i, p_own[i], self._erows[i, 1:2])
+                ops.dot(i, self.own(phi[i], i), self.own(x[i], i), self._erows[i, 2:3])
+            self.comm.reduce(self._erows, 0, 3, self._es)
+            e = self._es.cpu()
+        return float(e[0]), float(e[1]), float(e[2])
+
+    def _kick(self, p_own, x, h):
+        """p -= h (dS_F/dtheta + dS_B/dtheta) on the owned slices."""
+        ops = self.ops
+        with self._stream():
+            self.force(x, self._fF)
+            for i in range(self.k):
+                ops.force_boson(i, self._fB[i])
+                ops.field_axpy(i, p_own[i], self.own(self._fF[i], i), -h)
+                ops.field_axpy(i, p_own[i], self.own(self._fB[i], i), -h)
+
+    def trajectory(self, theta_own, p_own, phi, nsteps, eps, cg_tol=1e-10, cg_max_iter=1000000):
+        """One leapfrog trajectory, in place on theta_own[i], p_own[i] (this process's slices, [nt_loc][2][L][L] float64,
+        contiguous); phi: extended pseudofermion tensors.  -> dict(H0, H1, cg_iters, converged), as hqmc_leapfrog_trajectory."""
+        ops = self.ops
+        if not hasattr(self, "_fF"):
+            with self._stream():
+                self._fF = [ops.new_field(i) for i in range(self.k)]
+                self._fB = [ops.new_field(i) for i in range(self.k)]
+                self._X = [ops.new_vec(i) for i in range(self.k)]
+        X, total, ok = self._X, 0, True
+
+        def solve():
+            nonlocal total, ok
+            it, _, conv = self.solve(phi, X, cg_tol, cg_max_iter)
+            total += it
+            ok = ok and conv
+
+        self.set_theta(theta_own)
+        solve()
+        H0 = sum(self.energies(p_own, phi, X))
+        self._kick(p_own, X, 0.5 * eps)
+        for n in range(nsteps):
+            with self._stream():
+                for i in range(self.k):
+                    ops.field_axpy(i, theta_own[i], p_own[i], 2.0 * eps)          # theta += 2 p eps
+            self.set_theta(theta_own)
+            solve()
+            self._kick(p_own, X, 0.5 * eps if n == nsteps - 1 else eps)
+        H1 = sum(self.energies(p_own, phi, X))
+        return dict(H0=H0, H1=H1, cg_iters=total, converged=ok)

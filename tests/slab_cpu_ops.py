@@ -43,6 +43,25 @@ class OracleSlabOps:
     def force(self, i, x, out):
         out.copy_(torch.from_numpy(self.o[i].force_fermion(self.theta[i], x.numpy())))
 
+    def force_boson(self, i, out):
+        out.copy_(torch.from_numpy(self.o[i].force_boson(self.theta[i])))
+
+    def field_axpy(self, i, y, x, a):
+        y += a * x
+
+    def action_boson(self, i, first, count, out):
+        """The share of S_B of the slices [first, first + count): plaquettes of those slices and the temporal terms t -> t + 1."""
+        th = self.theta[i]
+        P = self.o[i].P
+        tx, ty = th[first:first + count, 0], th[first:first + count, 1]
+        curl = tx + np.roll(ty, -1, axis=2) - np.roll(tx, -1, axis=1) - ty          # theta_x(s) + theta_y(s+x) - theta_x(s+y) - theta_y(s)
+        d = th[first + 1:first + count + 1] - th[first:first + count]
+        temporal = (1.0 - np.cos(d)).sum() if P.compact else (d * d).sum()
+        out[0] = float(P.c_tau * temporal + P.K * np.cos(curl).sum())
+
+    def sum_squares(self, i, f, out):
+        out[0] = float((f.numpy() ** 2).sum())
+
     def dot(self, i, a, b, out):
         out[0] = float(np.vdot(a.numpy().ravel(), b.numpy().ravel()).real)
 

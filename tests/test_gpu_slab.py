@@ -93,6 +93,35 @@ def test_slab_pcg_equals_the_oracles_and_the_one_context_solve(cuda_device, S):
     g.close(); ops.close()
 
 
+@pytest.mark.parametrize("S,compact", [(1, True), (2, True), (3, False)])
+def test_slab_trajectory_dH_and_reversibility(cuda_device, S, compact):
+    """Leapfrog trajectory on the sharded lattice against the oracle's (Eq.16): H0, dH <= 1e-8, theta' <= 1e-10,
+    p' <= 1e-9, and the reversed trajectory returns to the start to <= 1e-10 (tight solves, reading C17)."""
+    L, Nt, W, nsteps, eps = 6, 26, 6, 4, 0.05
+    theta, p = inputs.theta_uniform(L, Nt, 23), inputs.momenta(L, Nt, 23)
+    eta = inputs.complex_gaussian((Nt, L, L), 23)
+    kw = dict(compact=compact, c_tau=0.8, K=1.2)
+    o = orc.Oracle(L, Nt, W=W, **kw)
+    phi = o.apply_Mdag(theta, eta)
+    ref = o.trajectory(theta, p, phi, nsteps, eps, cg_tol=1e-13)
+    lay = SlabLayout(L, Nt, S, W=W)
+    ops = CudaSlabOps(lay, **kw)
+    sol = SlabSolver(lay, ops)
+    th_own, p_own = parts(theta, lay), parts(p, lay)
+    phis = sol.extend(parts(phi, lay), ops.new_vec)
+    r = sol.trajectory(th_own, p_own, phis, nsteps, eps, cg_tol=1e-13)
+    assert r["converged"]
+    assert abs(r["H0"] - ref["H0"]) <= 1e-8 and abs((r["H1"] - r["H0"]) - (ref["H1"] - ref["H0"])) <= 1e-8
+    th = np.concatenate([t.cpu().numpy() for t in th_own]); pp = np.concatenate([t.cpu().numpy() for t in p_own])
+    assert np.abs(th - ref["theta"]).max() <= 1e-10 and np.abs(pp - ref["p"]).max() <= 1e-9 * max(1.0, np.abs(ref["p"]).max())
+    for t in p_own:
+        t.neg_()
+    sol.trajectory(th_own, p_own, phis, nsteps, eps, cg_tol=1e-13)
+    th = np.concatenate([t.cpu().numpy() for t in th_own]); pp = np.concatenate([t.cpu().numpy() for t in p_own])
+    assert np.abs(th - theta).max() <= 1e-10 and np.abs(pp + p).max() <= 1e-10 * max(1.0, np.abs(p).max())
+    ops.close()
+
+
 def test_config2_solve_in_four_slabs(cuda_device):
     """BASELINE config 2 (L=12, Ntau=120, heat-bath theta) solved to 1e-10 in four slabs of 30 slices."""
     c = inputs.CONFIGS[2]

@@ -72,6 +72,28 @@ def test_slab_operators_and_pcg_equal_the_global_ones(S, W):
     assert it == it9 == 9 and rel(gather(xs, lay, sol), x9) <= 1e-12 and abs(relres - rel9) <= 1e-10 * rel9
 
 
+@pytest.mark.parametrize("S,compact", [(1, True), (3, True), (2, False)])
+def test_slab_trajectory_equals_the_oracles(S, compact):
+    """Leapfrog trajectory on the sharded lattice (drift, extended theta with the neighbours' slices, sharded solve, fermion and
+    boson force, energies summed over owned slices) against the oracle's trajectory (PAPER.md:207-214 Eq.16, :181 Eq.12)."""
+    L, Nt, W = 4, 24, 4
+    theta, p = inputs.theta_uniform(L, Nt, 5), inputs.momenta(L, Nt, 5)
+    eta = inputs.complex_gaussian((Nt, L, L), 5)
+    o = orc.Oracle(L, Nt, W=W, compact=compact, c_tau=0.7, K=1.3)
+    phi = o.apply_Mdag(theta, eta)
+    ref = o.trajectory(theta, p, phi, 3, 0.05, cg_tol=1e-13)
+    lay = SlabLayout(L, Nt, S, W=W)
+    ops = OracleSlabOps(lay, compact=compact, c_tau=0.7, K=1.3)
+    sol = SlabSolver(lay, ops)
+    th_own = [t.clone() for t in parts(theta, lay)]
+    p_own = [t.clone() for t in parts(p, lay)]
+    r = sol.trajectory(th_own, p_own, sol.extend(parts(phi, lay), ops.new_vec), 3, 0.05, cg_tol=1e-13)
+    assert r["converged"] and abs(r["cg_iters"] - ref["cg_iters"]) <= 8
+    assert abs(r["H0"] - ref["H0"]) <= 1e-9 and abs((r["H1"] - r["H0"]) - (ref["H1"] - ref["H0"])) <= 1e-9
+    assert np.abs(np.concatenate([t.numpy() for t in th_own]) - ref["theta"]).max() <= 1e-11
+    assert np.abs(np.concatenate([t.numpy() for t in p_own]) - ref["p"]).max() <= 1e-10
+
+
 WORKER = r'''
 import os, sys
 sys.path.insert(0, sys.argv[1])
@@ -102,8 +124,14 @@ xs = [ops.new_vec(i) for i in range(len(lay.owned))]
 it, relres, conv = sol.solve(sol.extend(part(phi), ops.new_vec), xs, 1e-10, 5000)
 x_ref, it_ref, _ = o.pcg(theta, phi, 1e-10, 5000)
 e_x = max(float(np.abs(sol.own(xs[i], i).numpy() - x_ref[lay.bounds[g]:lay.bounds[g + 1]]).max()) for i, g in enumerate(lay.owned))
+p = inputs.momenta(L, Nt, 11)
+tr = o.trajectory(theta, p, phi, 2, 0.05, cg_tol=1e-13)
+th_own, p_own = [v.clone() for v in part(theta)], [v.clone() for v in part(p)]
+r = sol.trajectory(th_own, p_own, sol.extend(part(phi), ops.new_vec), 2, 0.05, cg_tol=1e-13)
+e_th = max(float(np.abs(th_own[i].numpy() - tr["theta"][lay.bounds[g]:lay.bounds[g + 1]]).max()) for i, g in enumerate(lay.owned))
+e_H = max(abs(r["H0"] - tr["H0"]), abs((r["H1"] - r["H0"]) - (tr["H1"] - tr["H0"])))
 dist.barrier()
-print(f"RESULT {rank} {e_op / np.abs(ref).max():.3e} {e_x / np.abs(x_ref).max():.3e} {it} {it_ref} {int(conv)}")
+print(f"RESULT {rank} {e_op / np.abs(ref).max():.3e} {e_x / np.abs(x_ref).max():.3e} {it} {it_ref} {int(conv)} {e_th:.3e} {e_H:.3e}")
 dist.destroy_process_group()
 '''
 
@@ -111,7 +139,7 @@ dist.destroy_process_group()
 @pytest.mark.parametrize("S", [2, 4])
 def test_slab_pcg_gloo_world2(tmp_path, S):
     """N>1 path: two processes, one or two slabs each, halos and sums over gloo; every rank's slices of M^+M v and of the PCG
-    solution equal the oracle's global result."""
+    solution equal the oracle's global result, and so does a two-step leapfrog trajectory (theta', H0, dH)."""
     script = tmp_path / "slab_worker.py"
     script.write_text(WORKER)
     port = 29600 + (os.getpid() % 300) + S
@@ -126,7 +154,8 @@ def test_slab_pcg_gloo_world2(tmp_path, S):
     for out, _ in outs:
         for line in out.splitlines():
             if line.startswith("RESULT"):
-                _, rank, e_op, e_x, it, it_ref, conv = line.split()
+                _, rank, e_op, e_x, it, it_ref, conv, e_th, e_H = line.split()
                 assert float(e_op) <= 1e-14 and float(e_x) <= 1e-9 and abs(int(it) - int(it_ref)) <= 2 and conv == "1"
+                assert float(e_th) <= 1e-11 and float(e_H) <= 1e-9            # the trajectory: theta' and H0, dH on every rank
                 seen += 1
     assert seen == 2
