@@ -291,6 +291,15 @@ def run_gpu(args):
     it_bytes = sum(bps.values()) * N
     roofline["iteration"] = {"alg_bytes_per_site": sum(bps.values()), "achieved": it_bytes / kern["iter_us"] / 1e3, "unit": "GB/s",
                              "frac": it_bytes / kern["iter_us"] / 1e3 / peak}
+    # the same kernel against the fp64 issue rate, the roof it actually sits under (DRAM 16 % busy): ~150
+    # flop per site and M^+M (two B products of 28 FMA per site, the link decode, the two axpys, the dot), peak = SMs x 64
+    # fp64 lanes x 2 flop x the SM clock sampled during the run
+    if dom == "mdagm" and prec == "c128":
+        sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+        alu_peak = torch.cuda.get_device_properties(0).multi_processor_count * 64 * 2 * sm_mhz * 1e6 / 1e12
+        alu_ach = 150.0 * N / (per_kernel[dom]["us_in_graph"] * 1e-6) / 1e12
+        roofline["alu"] = {"bound": "alu", "flops_per_site": 150, "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s",
+                           "frac": alu_ach / alu_peak, "peak_source": "SMs x 64 fp64 lanes x 2 x sampled SM clock (guide: unit counts)"}
     ms_per_step = ms / args.steps
     us_per_iter = kern["iter_us"]
     cb_dt, cb_apps, cb_threads = oracle_step_sample(L, Ntau, c["seed"], args.ref_cg_iters)
