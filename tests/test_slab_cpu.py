@@ -142,7 +142,7 @@ def test_slab_pcg_gloo_world2(tmp_path, S):
     solution equal the oracle's global result, and so does a two-step leapfrog trajectory (theta', H0, dH)."""
     script = tmp_path / "slab_worker.py"
     script.write_text(WORKER)
-    port = 29600 + (os.getpid() % 300) + S
+    port = 30100 + (os.getpid() % 300) + S
     procs = []
     for rank in range(2):
         env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), OMP_NUM_THREADS="1")
