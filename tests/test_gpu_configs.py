@@ -223,6 +223,20 @@ def test_persistent_pcg_kernel_selection_and_limits(hq):
     assert out[hq.PERSIST_OFF][2] >= 4 * 30
     assert rel(out[hq.PERSIST_ON][0].cpu().numpy(), out[hq.PERSIST_OFF][0].cpu().numpy()) <= 1e-12
     g.close()
+    # the largest lattice AUTO takes (L=20, Ntau=200: 200 CTAs of 128 threads, two per SM on some SMs): fixed-count iterates
+    L2, Nt2 = 20, 200
+    th2 = inputs.theta_uniform(L2, Nt2, 9)
+    v2 = inputs.complex_gaussian((Nt2, L2, L2), 9)
+    o2 = orc.Oracle(L2, Nt2)
+    orc.set_threads(orc.max_threads())
+    g = hq.HQMC(L2, Nt2)
+    g.set_theta(dev(th2))
+    g.reset_stats()
+    x, it, relres, _ = g.cg_solve(dev(v2), 0.0, 30)
+    xo, ito, relo = o2.pcg(th2, v2, 0.0, 30)
+    assert sum(v[0] for v in g.kernel_stats().values()) == 1 and it == ito == 30
+    assert rel(x.cpu().numpy(), xo) <= 1e-11 and abs(relres - relo) <= 1e-9 * relo
+    g.close()
     big = hq.HQMC(48, 20)
     with pytest.raises(hq.HqmcError):
         big.set_cg_persistent(hq.PERSIST_ON)
