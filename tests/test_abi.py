@@ -47,6 +47,12 @@ def test_argument_validation_and_no_cpu_fallback():
     bad = hqmc._Params(4, 8, 0.1, 1.0, 1.0, 1.0, 1, 8, 0)       # W >= Ntau
     assert lib.hqmc_create(C.byref(bad), None, C.byref(ctx)) == hqmc.HQMC_EINVAL
     assert lib.hqmc_apply_M(None, None, None) == hqmc.HQMC_EINVAL
+    for fn in (lib.hqmc_slab_dot, lib.hqmc_slab_axpy, lib.hqmc_slab_dupdate, lib.hqmc_slab_scale, lib.hqmc_slab_sum_rows,
+               lib.hqmc_slab_field_axpy, lib.hqmc_slab_action_boson, lib.hqmc_set_cg_persistent):
+        fn.argtypes = None
+    assert lib.hqmc_slab_dot(None, None, None, C.c_longlong(0), None) == hqmc.HQMC_EINVAL
+    assert lib.hqmc_slab_action_boson(None, 0, 1, None) == hqmc.HQMC_EINVAL
+    assert lib.hqmc_set_cg_persistent(None, 0) == hqmc.HQMC_EINVAL
     if not torch.cuda.is_available():
         ok = hqmc._Params(4, 8, 0.1, 1.0, 1.0, 1.0, 1, 6, 0)
         assert lib.hqmc_create(C.byref(ok), None, C.byref(ctx)) == hqmc.HQMC_ECUDA
