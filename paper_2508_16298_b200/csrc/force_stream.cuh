@@ -10,8 +10,9 @@
 //  * the links come as 8-byte packed phases (TMA, one slice ahead) and are decoded in the kernel, as in k_mdagm_back;
 //  * the eight bond sums of a thread go through the (then idle) exchange buffers into the slice's own [mu][y][x] order, so the
 //    epilogue -- dS_F/dtheta, or the kick with the bosonic force from the link-phase table -- reads p and the phases and
-//    writes p in full lines.  (Pulling those lines into L2 a step ahead with prefetch.global.L2 was measured: 78 vs 70 us,
-//    the prefetches compete with the TMA loads.)
+//    writes p in full lines.  What the epilogue reads for the first time (the phases of slice t-1, p of slice t) is pulled into
+//    L2 by two bulk prefetches the leader issues at the start of the step: 70 -> 66 us in situ.  (Per-thread prefetch.global.L2
+//    instructions a step ahead had lost, 78 us: they compete with the sweeps for the LSU.)
 // Slices are addressed by n = t1 - t (n = 0: the halo slice t1); slice n lives in X buffer n mod 2.
 #pragma once
 #include "force_kernels.cuh"
@@ -151,7 +152,16 @@ __global__ void __launch_bounds__(576, 1) k_force_stream(Geo g, const typename P
         T2 r0, r1, r2, r3;
         load_block_swz(reinterpret_cast<const T2 *>(xb(n)), b, r0, r1, r2, r3);
         // forward: R = prod_k (1 + T_k) X_t.  Behind its first barrier every thread has decoded the links: fetch the next ones.
-        lean_apply_B2(ex, nbp, b, P, r0, r1, r2, r3, [&]() { if (leader && n + 1 <= nsl) load_p(n + 1); }, []() {});
+        lean_apply_B2(ex, nbp, b, P, r0, r1, r2, r3, [&]() {
+            if (leader) {
+                if (n + 1 <= nsl) load_p(n + 1);
+                if (FUSE_P) {      // what this step's epilogue will read for the first time: into L2 while the sweeps run
+                    const int tpp = (t == 0) ? g.Nt - 1 : t - 1;
+                    if (PHASE_BOSON && compact) bulk_prefetch_l2(ph + (size_t)tpp * 2 * g.Vs, (uint32_t)(2 * g.Vs * sizeof(T2)));
+                    bulk_prefetch_l2(out + (size_t)t * 2 * g.Vs, (uint32_t)(2 * g.Vs * sizeof(double)));
+                }
+            }
+        }, []() {});
         // (the barriers of the forward product separate the previous step's reads of Splaq from these writes)
         if (PHASE_BOSON) force_splaq(g, ph + (size_t)t * 2 * g.Vs, Splaq, i_half, i_full);
         T2 l0, l1, l2, l3;                                    // Y_{t+1} = X_{t+1} - sigma C R
