@@ -136,16 +136,17 @@ dist.destroy_process_group()
 '''
 
 
-@pytest.mark.parametrize("S", [2, 4])
-def test_slab_pcg_gloo_world2(tmp_path, S):
-    """N>1 path: two processes, one or two slabs each, halos and sums over gloo; every rank's slices of M^+M v and of the PCG
+@pytest.mark.parametrize("world,S", [(2, 2), (2, 4), (3, 3)])
+def test_slab_pcg_gloo(tmp_path, world, S):
+    """N>1 path: two processes with one or two slabs each (both neighbours of a rank are the same peer) and three processes
+    (distinct peers below and above), halos and sums over gloo; every rank's slices of M^+M v and of the PCG
     solution equal the oracle's global result, and so does a two-step leapfrog trajectory (theta', H0, dH)."""
     script = tmp_path / "slab_worker.py"
     script.write_text(WORKER)
-    port = 30100 + (os.getpid() % 300) + S
+    port = 30100 + (os.getpid() % 300) + 10 * world + S
     procs = []
-    for rank in range(2):
-        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), OMP_NUM_THREADS="1")
+    for rank in range(world):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), OMP_NUM_THREADS="1")
         procs.append(subprocess.Popen([sys.executable, str(script), ROOT, str(port), str(S)], env=env, stdout=subprocess.PIPE,
                                       stderr=subprocess.PIPE, text=True))
     outs = [p.communicate(timeout=300) for p in procs]
@@ -158,4 +159,4 @@ def test_slab_pcg_gloo_world2(tmp_path, S):
                 assert float(e_op) <= 1e-14 and float(e_x) <= 1e-9 and abs(int(it) - int(it_ref)) <= 2 and conv == "1"
                 assert float(e_th) <= 1e-11 and float(e_H) <= 1e-9            # the trajectory: theta' and H0, dH on every rank
                 seen += 1
-    assert seen == 2
+    assert seen == world
