@@ -163,6 +163,15 @@ int hqmc_sweep(hqmc_ctx *ctx, double *d_theta, unsigned long long seed, unsigned
                double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out, int *accepted_out,
                long long *cg_iters_out);
 
+/* The same sweep for n_chain independent chains advanced together (hqmc_hqmc_step_batched per update): d_theta
+ * [n_chain][Ntau][2][L][L] in/out; chain b draws exactly what hqmc_sweep would draw from seed + b (same counters and streams,
+ * update index first_update + k), so a batched sweep is reproducible chain by chain.  H0_out, H1_out, accepted_out,
+ * cg_iters_out: HOST arrays of n_updates * n_chain entries, update-major ([k][b]); any may be NULL.  The eta and p workspace is
+ * allocated for the call and freed before it returns (synchronises the stream). */
+int hqmc_sweep_batched(hqmc_ctx *ctx, double *d_theta, unsigned long long seed, unsigned first_update, int n_updates, int n_chain,
+                       int nsteps, double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
+                       int *accepted_out, long long *cg_iters_out);
+
 /* ---- Stochastic estimation of fermionic observables ----
  * All pointers are DEVICE pointers to lattice vectors [Ntau][L][L] of the context's complex type (n_rv of them back to
  * back where a count is given), 16-byte aligned, caller-owned.  The calls enqueue on the context's stream; cuFFT provides

@@ -184,3 +184,37 @@ extern "C" int hqmc_hqmc_step_batched(hqmc_ctx *c, double *d_theta, double *d_p,
     if (any_rej) CUDA_TRY(cudaStreamSynchronize(c->stream));
     return s;
 }
+
+// n_updates HQMC updates of n_chain independent chains with every random number drawn on the device: chain b
+// is the chain hqmc_sweep would run from seed + b (same counters, key shifted by b), its updates advanced together with the other
+// chains' by hqmc_hqmc_step_batched.
+extern "C" int hqmc_sweep_batched(hqmc_ctx *c, double *d_theta, unsigned long long seed, unsigned first_update, int n_updates, int n_chain,
+                                  int nsteps, double eps, double cg_tol, long long cg_max_iter, double *H0_out, double *H1_out,
+                                  int *accepted_out, long long *cg_iters_out) {
+    if (!c || !aligned16(d_theta) || n_updates < 0 || n_chain < 1 || nsteps < 0 || cg_max_iter < 0) return HQMC_EINVAL;
+    void *d_eta = nullptr; double *d_p = nullptr;
+    CUDA_TRY(cudaMalloc(&d_eta, (size_t)n_chain * c->N * c->esz));
+    if (cudaMalloc((void **)&d_p, (size_t)n_chain * 2 * c->N * sizeof(double)) != cudaSuccess) { cudaFree(d_eta); g_last_error = "cudaMalloc"; return HQMC_ENOMEM; }
+    std::vector<double> u((size_t)n_chain);
+    int worst = HQMC_OK, st = HQMC_OK;
+    for (int k = 0; k < n_updates && st == HQMC_OK; ++k) {
+        const uint32_t upd = (uint32_t)first_update + (uint32_t)k;
+        for (int b = 0; b < n_chain && st == HQMC_OK; ++b) {
+            const unsigned long long sb = seed + (unsigned long long)b;
+            void *eb = (char *)d_eta + (size_t)b * c->N * c->esz;
+            if (c->prm.prec == HQMC_C128) st = launch(c, HQMC_K_MISC, k_rng<double, 2>, dim3(rng_grid(c, c->N)), dim3(256), 0, sb, upd, 0u, c->N, eb);
+            else st = launch(c, HQMC_K_MISC, k_rng<float, 2>, dim3(rng_grid(c, c->N)), dim3(256), 0, sb, upd, 0u, c->N, eb);
+            if (st == HQMC_OK)
+                st = launch(c, HQMC_K_MISC, k_rng<double, 1>, dim3(rng_grid(c, c->N)), dim3(256), 0, sb, upd, 1u, c->N, (void *)(d_p + (size_t)b * 2 * c->N));
+            u[b] = hqmc_rng_uniform(sb, upd);
+        }
+        if (st != HQMC_OK) break;
+        const size_t o = (size_t)k * n_chain;
+        st = hqmc_hqmc_step_batched(c, d_theta, d_p, d_eta, u.data(), n_chain, nsteps, eps, cg_tol, cg_max_iter, H0_out ? H0_out + o : nullptr,
+                                    H1_out ? H1_out + o : nullptr, accepted_out ? accepted_out + o : nullptr, cg_iters_out ? cg_iters_out + o : nullptr);
+        if (st == HQMC_ENOCONV) { worst = st; st = HQMC_OK; }
+    }
+    cudaStreamSynchronize(c->stream);
+    cudaFree(d_eta); cudaFree(d_p);
+    return st != HQMC_OK ? st : worst;
+}

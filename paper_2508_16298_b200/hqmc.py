@@ -26,7 +26,7 @@ KERNEL_CLASSES = ["mdagm", "cg_axpy", "precond", "cg_dupdate", "apply_M", "force
 SYMBOLS = [
     "hqmc_create", "hqmc_destroy", "hqmc_set_precond", "hqmc_get_precond", "hqmc_set_theta", "hqmc_apply_M",
     "hqmc_apply_Mdag", "hqmc_apply_MdagM", "hqmc_precond", "hqmc_cg_solve", "hqmc_force", "hqmc_force_boson",
-    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_rng_raw", "hqmc_rng_gauss", "hqmc_rng_uniform", "hqmc_sweep", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
+    "hqmc_energies", "hqmc_leapfrog_trajectory", "hqmc_hqmc_step", "hqmc_rng_raw", "hqmc_rng_gauss", "hqmc_rng_uniform", "hqmc_sweep", "hqmc_sweep_batched", "hqmc_cg_solve_batched", "hqmc_leapfrog_trajectory_batched", "hqmc_refresh_batched", "hqmc_hqmc_step_batched", "hqmc_set_green_batch", "hqmc_green_apply", "hqmc_translation_average", "hqmc_green_2pt",
     "hqmc_pair_correlator", "hqmc_apply_MdagM_host", "hqmc_refresh_host", "hqmc_cg_solve_host",
     "hqmc_leapfrog_trajectory_host", "hqmc_action_boson_noalloc", "hqmc_slab_dot", "hqmc_slab_axpy", "hqmc_slab_dupdate",
     "hqmc_slab_scale", "hqmc_slab_sum_rows", "hqmc_slab_field_axpy", "hqmc_slab_action_boson", "hqmc_set_profiling", "hqmc_reset_stats", "hqmc_get_kernel_stats",
@@ -238,6 +238,18 @@ class HQMC:
                                    C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter), H0, H1, acc, it),
                    allow_noconv=True)
         return dict(H0=list(H0), H1=list(H1), accepted=[bool(a) for a in acc], cg_iters=list(it), converged=(s == HQMC_OK))
+
+    def sweep_batched(self, theta, seed, first_update, n_updates, nsteps, eps, cg_tol=1e-10, cg_max_iter=1000000):
+        """n_updates HQMC updates of the n chains stacked in theta [n][Ntau][2][L][L] (in place); chain b draws what `sweep` draws
+        from seed + b -> dict(H0, H1, accepted, cg_iters: lists [update][chain], converged)."""
+        assert theta.is_cuda and theta.dtype == torch.float64 and theta.is_contiguous() and theta.numel() % (2 * self.N) == 0
+        n, m = theta.numel() // (2 * self.N), n_updates
+        H0, H1, it, acc = (C.c_double * (n * m))(), (C.c_double * (n * m))(), (C.c_longlong * (n * m))(), (C.c_int * (n * m))()
+        s = _check(_lib.hqmc_sweep_batched(self._ctx, _ptr(theta), C.c_ulonglong(seed), C.c_uint(first_update), C.c_int(m), C.c_int(n),
+                                           C.c_int(nsteps), C.c_double(eps), C.c_double(cg_tol), C.c_longlong(cg_max_iter), H0, H1, acc, it),
+                   allow_noconv=True)
+        rows = lambda a, f: [[f(a[k * n + b]) for b in range(n)] for k in range(m)]
+        return dict(H0=rows(H0, float), H1=rows(H1, float), accepted=rows(acc, bool), cg_iters=rows(it, int), converged=(s == HQMC_OK))
 
     # ---- stochastic estimator (PAPER.md:220-244) -------------------------------------------------
     def _vecs(self, v):

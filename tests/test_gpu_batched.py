@@ -203,3 +203,27 @@ def test_batched_hqmc_step_accepts_and_rejects_per_chain(hq):
             assert np.array_equal(TH[b], thetas[b]), b
         assert np.abs(P[b] - ref["p"]).max() <= 1e-10, b
     g.close()
+
+
+def test_batched_sweep_equals_the_oracles_sweep_chain_by_chain(hq):
+    """hqmc_sweep_batched (every draw on the device, chain b keyed by seed + b): acceptance sequences, H0, dH and
+    the final theta of every chain equal the oracle's one-chain sweep from seed + b."""
+    L, Nt, seed, n_upd, n_chain = 6, 10, 99, 4, 3
+    thetas = np.stack([inputs.theta_uniform(L, Nt, 1 + b) for b in range(n_chain)])
+    o = orc.Oracle(L, Nt, c_tau=0.0, K=0.0)
+    g = hq.HQMC(L, Nt, c_tau=0.0, K=0.0)
+    refs = [o.hqmc_sweep(thetas[b], seed + b, 3, n_upd, 5, 0.2, cg_tol=1e-13) for b in range(n_chain)]
+    dth = dev(thetas)
+    r = g.sweep_batched(dth, seed, 3, n_upd, 5, 0.2, cg_tol=1e-13)
+    assert r["converged"]
+    out = dth.cpu().numpy()
+    n_acc = 0
+    for b in range(n_chain):
+        acc = [r["accepted"][k][b] for k in range(n_upd)]
+        assert acc == list(refs[b]["accepted"]), (b, acc, refs[b]["accepted"])
+        n_acc += sum(acc)
+        H0 = np.array([r["H0"][k][b] for k in range(n_upd)]); H1 = np.array([r["H1"][k][b] for k in range(n_upd)])
+        assert np.abs(H0 - refs[b]["H0"]).max() <= 1e-8 and np.abs((H1 - H0) - (refs[b]["H1"] - refs[b]["H0"])).max() <= 1e-8
+        assert np.abs(out[b] - refs[b]["theta"]).max() <= 1e-9
+    assert 0 < n_acc < n_upd * n_chain                      # both branches of the Metropolis step were taken
+    g.close()
