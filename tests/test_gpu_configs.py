@@ -115,6 +115,31 @@ def test_config3_twenty_step_trajectory_dH_and_reversibility(hq):
     g.close()
 
 
+def test_twenty_step_trajectory_with_converged_solves(hq):
+    """Config 3's protocol (20 leapfrog steps, uniform theta) with CONVERGED solves, where it is a stable integration: L=8, Ntau=80,
+    eps = 0.005 (at config 3's eps = 0.05 the leapfrog diverges on both sides).  21 solves of ~1000 iterations to
+    1e-12 on each side: H0, dH, theta', p' and the reversed trajectory (reading C17)."""
+    L, Nt, nsteps, eps = 8, 80, 20, 0.005
+    theta, p = inputs.theta_uniform(L, Nt, 2), inputs.momenta(L, Nt, 2)
+    eta = inputs.complex_gaussian((Nt, L, L), 2)
+    o = orc.Oracle(L, Nt)
+    orc.set_threads(orc.max_threads())
+    phi = o.apply_Mdag(theta, eta)
+    ref = o.trajectory(theta, p, phi, nsteps, eps, cg_tol=1e-12, cg_max_iter=1000000)
+    g = hq.HQMC(L, Nt)
+    dth, dp, dphi = dev(theta), dev(p), dev(phi)
+    r = g.trajectory(dth, dp, dphi, nsteps, eps, cg_tol=1e-12, cg_max_iter=1000000)
+    assert r["converged"] and abs(r["cg_iters"] - ref["cg_iters"]) <= max(21 * 2, ref["cg_iters"] // 100)
+    bound = 1e-8 * max(1.0, abs(ref["H0"]) * 1e-6) * 10          # 21 solves at 1e-12 each
+    assert abs(r["H0"] - ref["H0"]) <= bound and abs((r["H1"] - r["H0"]) - (ref["H1"] - ref["H0"])) <= 1e-6
+    assert np.abs(dth.cpu().numpy() - ref["theta"]).max() <= 1e-9
+    assert np.abs(dp.cpu().numpy() - ref["p"]).max() <= 1e-7 * max(1.0, np.abs(ref["p"]).max())
+    dp.neg_()
+    g.trajectory(dth, dp, dphi, nsteps, eps, cg_tol=1e-12, cg_max_iter=1000000)
+    assert np.abs(dth.cpu().numpy() - theta).max() <= 1e-8 and np.abs(dp.cpu().numpy() + p).max() <= 1e-6 * max(1.0, np.abs(p).max())
+    g.close()
+
+
 def test_config4_converged_solve_judged_by_the_oracles_operator(hq):
     """Config 4 (L=48, Ntau=480, uniform theta): preconditioned CG to 1e-10 (about 3e5 iterations, some 20 s on the GPU;
     far out of the oracle's reach), then ONE oracle M^+M: ||phi - O_oracle x_gpu|| / ||phi|| <= 1.05e-10 (reading C16 i)."""
