@@ -140,6 +140,33 @@ def test_twenty_step_trajectory_with_converged_solves(hq):
     g.close()
 
 
+@pytest.mark.parametrize("L,Nt", [(8, 80), (12, 60)])
+def test_paper_regime_trajectory_with_converged_solves(hq, L, Nt):
+    """The regime the method is run in (c_tau = 1/(J dtau^2) = 80, K = 1; smooth-in-tau fields, O(100) PCG iterations):
+    a 10-step trajectory at eps = 0.02 (c_tau = 80 puts the leapfrog's stability edge near 0.05) with solves converged to 1e-12 on both sides, c_tau = 80 in the bosonic force and action:
+    H0, dH, theta', p', reversibility."""
+    nsteps, eps, kw = 10, 0.02, dict(c_tau=80.0, K=1.0)
+    theta = inputs.theta_paper_regime(L, Nt, 6, sweeps=20)
+    p, eta = inputs.momenta(L, Nt, 6), inputs.complex_gaussian((Nt, L, L), 6)
+    o = orc.Oracle(L, Nt, **kw)
+    orc.set_threads(orc.max_threads())
+    phi = o.apply_Mdag(theta, eta)
+    ref = o.trajectory(theta, p, phi, nsteps, eps, cg_tol=1e-12, cg_max_iter=100000)
+    g = hq.HQMC(L, Nt, **kw)
+    dth, dp, dphi = dev(theta), dev(p), dev(phi)
+    r = g.trajectory(dth, dp, dphi, nsteps, eps, cg_tol=1e-12, cg_max_iter=100000)
+    assert r["converged"] and abs(r["cg_iters"] - ref["cg_iters"]) <= max(22, ref["cg_iters"] // 100)
+    assert abs(ref["H1"] - ref["H0"]) < 50.0                     # a stable integration, not a divergence
+    assert abs(r["H0"] - ref["H0"]) <= 1e-8 * max(1.0, abs(ref["H0"]) * 1e-6) * 10
+    assert abs((r["H1"] - r["H0"]) - (ref["H1"] - ref["H0"])) <= 1e-8
+    assert np.abs(dth.cpu().numpy() - ref["theta"]).max() <= 1e-10
+    assert np.abs(dp.cpu().numpy() - ref["p"]).max() <= 1e-9 * max(1.0, np.abs(ref["p"]).max())
+    dp.neg_()
+    g.trajectory(dth, dp, dphi, nsteps, eps, cg_tol=1e-12, cg_max_iter=100000)
+    assert np.abs(dth.cpu().numpy() - theta).max() <= 1e-10 and np.abs(dp.cpu().numpy() + p).max() <= 1e-10 * max(1.0, np.abs(p).max())
+    g.close()
+
+
 def test_config4_converged_solve_judged_by_the_oracles_operator(hq):
     """Config 4 (L=48, Ntau=480, uniform theta): preconditioned CG to 1e-10 (about 3e5 iterations, some 20 s on the GPU;
     far out of the oracle's reach), then ONE oracle M^+M: ||phi - O_oracle x_gpu|| / ||phi|| <= 1.05e-10 (reading C16 i)."""
