@@ -248,6 +248,7 @@ def test_leapfrog_step_graph_is_bitwise_identical_to_plain_launches(hq, L, Nt):
     out = []
     for on in (True, False):
         g = hq.HQMC(L, Nt)
+        g.set_cg_persistent(hq.PERSIST_OFF)          # (small lattices would take the one-launch solve and no step graph at all)
         g.set_md_graph(on)
         dth, dp = dev(theta), dev(p)
         r = g.trajectory(dth, dp, dev(phi), 4, 0.05, cg_tol=0.0, cg_max_iter=70)      # 70: not a multiple of the 32-iteration chunk
