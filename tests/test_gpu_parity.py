@@ -219,9 +219,11 @@ def test_complex64_variant(hq):
     out = g.apply_MdagM(dev(v.astype(np.complex64))).cpu().numpy().astype(np.complex128)
     ref = o.apply_MdagM(theta, v)
     assert np.linalg.norm((out - ref).ravel()) / np.linalg.norm(ref.ravel()) <= 1e-6
-    x, it, relres, _ = g.cg_solve(dev(v.astype(np.complex64)), 0.0, 50)
     xo, _, relo = o.pcg(theta, v, 0.0, 50)
-    assert it == 50 and np.linalg.norm((x.cpu().numpy() - xo).ravel()) / np.linalg.norm(xo.ravel()) <= 1e-3
+    for mode in (hq.PERSIST_OFF, hq.PERSIST_ON):            # the four-kernel loop and the one-launch kernel, both in complex64
+        g.set_cg_persistent(mode)
+        x, it, relres, _ = g.cg_solve(dev(v.astype(np.complex64)), 0.0, 50)
+        assert it == 50 and np.linalg.norm((x.cpu().numpy() - xo).ravel()) / np.linalg.norm(xo.ravel()) <= 1e-3, mode
     g.close()
 
 
