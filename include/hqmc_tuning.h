@@ -64,8 +64,8 @@ int hqmc_set_green_batch(hqmc_ctx *ctx, int n);
 int hqmc_set_md_graph(hqmc_ctx *ctx, int on);
 
 /* Programmatic dependent launch inside the PCG iteration (kernel k+1 is dispatched under kernel k's tail and waits
- * on-device for its completion before reading its output). 1 (default) = the preconditioner and the d update, the two
- * launches that follow a kernel filling every SM; 0 = off; 16 + mask = per-kernel-class mask (bit = HQMC_K_* class),
+ * on-device for its completion before reading its output). 1 (default) = every launch of the iteration up to L = 44, and at
+ * L >= 48 the preconditioner and the d update only, the two launches that follow a kernel filling every SM evenly; 0 = off; 16 + mask = per-kernel-class mask (bit = HQMC_K_* class),
  * for timing experiments. Results are bit-identical in every setting. */
 int hqmc_set_pdl(hqmc_ctx *ctx, int on);
 

@@ -146,6 +146,7 @@ extern "C" int hqmc_create(const hqmc_params *prm, void *cuda_stream, hqmc_ctx *
     st = build_default_taps(c);
     if (st != HQMC_OK) return fail(st);
     precond_cfg(c, 0);
+    c->pdl = pdl_default(c);
     {   // persistent whole-solve kernel: one CTA per slice, all of them resident at once (cooperative launch)
         int coop = 0, per_sm = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
@@ -279,7 +280,7 @@ extern "C" int hqmc_set_debug_skip(hqmc_ctx *c, unsigned mask) {
 }
 extern "C" int hqmc_set_pdl(hqmc_ctx *c, int on) {
     if (!c) return HQMC_EINVAL;
-    c->pdl = on == 1 ? HQMC_PDL_DEFAULT : (on >= 16 ? (on & 15) : 0);     // >= 16: per-class mask (timing experiments)
+    c->pdl = on == 1 ? pdl_default(c) : (on >= 16 ? (on & 15) : 0);     // >= 16: per-class mask (timing experiments)
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
     return HQMC_OK;
 }

@@ -143,6 +143,13 @@ struct hqmc_ctx {
     std::vector<hqmc::EventPair> pool;
 };
 
+// Default programmatic-launch mask: every edge of the iteration where the streaming M^+M CTA leaves room on its SM (up to 512 threads,
+// L <= 44: 2 % at L = 32...44, neutral below; measured, profiles/r02_summary.md), the two safe edges where it fills the SM (L = 48:
+// the early axpy CTAs pile up behind it, +6 us) and for the cluster / register kernels.
+static int pdl_default(const hqmc_ctx *c) {
+    return (c->use_stream && c->stream_on && c->cfg.threads <= 512) ? 15 : HQMC_PDL_DEFAULT;
+}
+
 // The PCG loop's live set is r, d, Od|z and the packed phases (4 x N x esz; x is streamed). While it fits the L2 the textbook
 // kernels win (their traffic is L2 traffic); beyond it the deferred-x pair, which moves 16 B/site less, does
 // (L=64, Ntau=640, 168 MB: 128.9 vs 131.5 us per iteration; L=48, Ntau=480, 71 MB: 53.2 vs 52.4; profiles/r01_summary.md).
