@@ -39,6 +39,31 @@ def test_layout_covers_the_lattice_once():
         SlabLayout(8, 10, 2, W=6)          # a slab shorter than the halo
 
 
+def test_layout_properties_on_random_shapes():
+    """Any admissible (Ntau, slabs, W, world): the slabs tile [0, Ntau) once, sizes differ by at most one, every process owns the
+    same number of consecutive slabs, and a slab's extended lattice is its slices with H slices of its neighbours either side."""
+    rng = np.random.default_rng(5)
+    seen = 0
+    for _ in range(300):
+        W = int(rng.integers(0, 9)); world = int(rng.integers(1, 5)); per = int(rng.integers(1, 4)); S = world * per
+        Nt = int(rng.integers(S * max(1, W), S * max(1, W) + 60))
+        lay = [SlabLayout(4, Nt, S, W=W, world=world, rank=r) for r in range(world)]
+        sizes = [lay[0].nt(g) for g in range(S)]
+        assert sum(sizes) == Nt and max(sizes) - min(sizes) <= 1 and min(sizes) >= lay[0].H
+        assert sorted(g for l in lay for g in l.owned) == list(range(S)) and all(len(l.owned) == per for l in lay)
+        covered = []
+        for g in range(S):
+            ext = lay[0].ext_slices(g)
+            H, n = lay[0].H, lay[0].nt(g)
+            assert len(ext) == n + 2 * H and ext[H:H + n] == list(range(lay[0].bounds[g], lay[0].bounds[g + 1]))
+            assert ext[:H] == [(lay[0].bounds[g] - H + j) % Nt for j in range(H)] and ext[H + n:] == [(lay[0].bounds[g + 1] + j) % Nt for j in range(H)]
+            assert lay[0].owner(g) == g // per
+            covered += ext[H:H + n]
+        assert covered == list(range(Nt))
+        seen += 1
+    assert seen == 300
+
+
 @pytest.mark.parametrize("S,W", [(1, 6), (2, 6), (3, 2), (4, 0)])
 def test_slab_operators_and_pcg_equal_the_global_ones(S, W):
     L, Nt = 4, 26
